@@ -1,0 +1,155 @@
+/* rips.h -- C ABI of the B200-native Vietoris-Rips hot path (arXiv 2003.07989, "Ripser++").
+ *
+ * Citations are lines of /root/reference/PAPER.md (the paper's text).  The library computes, per
+ * dimension d >= 1, the two stages of Fig. 3(b):
+ *
+ *   stage 1  filtration construction with clearing, Algorithms 7-8: every
+ *            candidate d-simplex by combinatorial index (Eq. 2), its diameter
+ *            (Eq. 1), keep iff diameter <= threshold and the simplex is not the
+ *            death simplex of a pair of dimension d-1 (clearing lemma), sorted
+ *            by diameter descending, index ascending;
+ *   stage 2  apparent pairs, Algorithm 3 / Lemma 7: per column s the
+ *            oldest cofacet t of equal diameter, and the test that s is the youngest facet of t;
+ *            the pairs (t, s) sorted by t with a binary-search lookup, the
+ *            non-apparent columns kept in coboundary order.
+ *
+ * Dimension 0 and the reduction of the non-apparent columns (Algorithm 2,
+ * PAPER.md:182-200) complete the barcodes; they are not the hot path and are timed separately
+ * (rips_timings).  Every step of stage 1 and stage 2 runs in hand-written CUDA kernels for
+ * sm_100a; there is no CPU fallback: on a machine without a usable CUDA device every entry point
+ * that needs the device returns RIPS_ECUDA.
+ *
+ * Conventions
+ *   - A d-simplex (v_d > ... > v_0 >= 0) has index cidx = sum_k C(v_k, k+1) (Eq. 2).
+ *   - Distance matrix: strict lower triangle, row-major, fp32; element (i > j) at i(i-1)/2 + j,
+ *     which is the cidx of the edge (i j).  -0.0f is canonicalised to +0.0f.
+ *   - All functions return 0 (RIPS_OK) or a negative error code; nothing throws or aborts.
+ *   - Pointers named *_dev are device pointers, *_host host pointers.  Every output array is
+ *     owned by the context and stays valid until the next call that recomputes it (rips_compute,
+ *     rips_stage1/2 for the same d) or rips_free.  The input matrix is copied by rips_init.
+ *   - All work is enqueued on the stream given to rips_init; calls that return host-visible
+ *     counts synchronise that stream.
+ *   - Not thread-safe per context; distinct contexts are independent.
+ */
+#ifndef RIPS_H
+#define RIPS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rips_ctx rips_ctx;
+
+enum {
+    RIPS_OK = 0,
+    RIPS_EINVAL = -1,    /* bad argument: n < 1, dim_max out of [0,4], NaN/negative/non-finite distance,
+                            NaN threshold, d out of range, stage called before its inputs exist */
+    RIPS_EOVERFLOW = -2, /* C(n, dim_max+3) >= 2^63, n >= 65536, or (rank bits + index bits) > 64 so a
+                            column does not fit the packed 64-bit record */
+    RIPS_ENOMEM = -3,    /* device or host allocation failed / caller's workspace too small */
+    RIPS_ECUDA = -4      /* CUDA runtime error; text via rips_last_error */
+};
+
+/* Counts per dimension d (Table 5's bookkeeping; Table 1). */
+typedef struct {
+    int64_t n_candidates;          /* C(n, d+1) */
+    int64_t n_removed_by_diameter; /* diameter > threshold */
+    int64_t n_cleared;             /* diameter <= threshold and cleared */
+    int64_t n_columns;             /* kept = length of the filtration array */
+    int64_t n_apparent;            /* apparent pairs found by stage 2 */
+    int64_t n_nonapparent;         /* columns left for the reduction */
+    int64_t n_reduced_pivots;      /* pairs found by the reduction */
+    int64_t n_essential;           /* columns that reduce to zero */
+    int64_t n_additions;           /* column additions performed by the reduction */
+    int64_t n_bars;                /* bars of non-zero length reported by rips_barcodes */
+    int32_t key_bits;              /* bits of the diameter rank inside a packed record */
+    int32_t index_bits;            /* bits of the combinatorial index inside a packed record */
+    int32_t sort_passes;           /* radix passes run by the filtration sort */
+    int32_t pair_sort_passes;      /* radix passes run by the pair sort */
+} rips_stats_t;
+
+/* Device time per step of dimension d, milliseconds, CUDA events on the library's stream
+ * (host-side pieces by a host clock).  Valid after the stream has been synchronised. */
+typedef struct {
+    float clear_bitmap_ms;   /* a4: clearing bitmap built from P_{d-1} */
+    float enumerate_ms;      /* a3-a5: enumerate + diameter + filter + ordered compaction */
+    float sort_hist_ms;      /* a6: digit histograms */
+    float sort_pass_ms;      /* a6: all onesweep passes */
+    float apparent_ms;       /* a7-a8: apparent-pair kernel with partition */
+    float pair_hist_ms;      /* a9 */
+    float pair_sort_ms;      /* a9 */
+    float stage1_ms;         /* whole stage 1 as enqueued (including memsets, scalar read-back) */
+    float stage2_ms;         /* whole stage 2 */
+    float dim0_ms;           /* d == 0 only: edge sort is part of rips_init; this is the union-find kernel */
+    float reduce_host_ms;    /* NOT hot path: serial reduction of non-apparent columns on the host */
+    float reduce_xfer_ms;    /* NOT hot path: D2H/H2D copies around the host reduction */
+} rips_timings_t;
+
+/* Exact upper bound, in bytes, of the device memory rips_compute needs for (n, dim_max) with no
+ * threshold (a threshold only lowers it).  RIPS_EOVERFLOW if the sizes do not fit. */
+int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes);
+
+/* Create a context.  dist_lower: n(n-1)/2 fp32, HOST or DEVICE pointer (detected), layout above.
+ * dim_max in [0,4]: H_0..H_dim_max.  threshold: keep simplices of diameter <= threshold
+ * (inclusive); +INFINITY = full complex; the library never substitutes the
+ * enclosing radius on its own.  stream: a cudaStream_t cast to void*, NULL = the
+ * default stream.  Validates the matrix (RIPS_EINVAL on NaN, negative or infinite entries), copies
+ * it, ranks the distinct edge values on the device and builds the binomial table.  */
+int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* stream);
+
+/* Dimension 0 .. dim_max, all stages: dim 0, then per d: stage 1, stage 2, reduction. */
+int rips_compute(rips_ctx* ctx);
+
+/* The two hot-path stages, separately callable for d in [1, dim_max+1] (benches, and the scale row
+ * of DESIGN.md: stage 1 at d = dim_max+1 enumerates the C(n, dim_max+2) simplices the configs
+ * name).  rips_stage1(d) needs the pivots of dimension d-1 (rips_compute, or rips_dim0 for d = 1);
+ * rips_stage2(d) needs rips_stage1(d).  Both may be called repeatedly. */
+int rips_dim0(rips_ctx* ctx);
+int rips_stage1(rips_ctx* ctx, int d);
+int rips_stage2(rips_ctx* ctx, int d);
+/* Reduction of the non-apparent columns of dimension d (after rips_stage2(d)); completes the pivots
+ * of dimension d.  Not the hot path: runs Algorithm 2 serially on the host, timed separately. */
+int rips_reduce(rips_ctx* ctx, int d);
+
+/* Bars of dimension d: 2*count floats (birth, death) on the HOST; death = +INFINITY for essential
+ * classes; zero-length bars omitted.  Order: d = 0: by ascending index of the merging edge, then
+ * the essential classes; d >= 1: column (coboundary) order of the birth simplex. */
+int rips_barcodes(rips_ctx* ctx, int d, const float** birth_death_host, int64_t* count);
+
+/* Filtration array C of dimension d >= 1 in coboundary order. */
+int rips_filtration(rips_ctx* ctx, int d, const float** diam_dev, const uint64_t** cidx_dev, int64_t* len);
+/* Apparent pairs of dimension d, ascending by cidx(t). */
+int rips_apparent_pairs(rips_ctx* ctx, int d, const uint64_t** t_dev, const uint64_t** s_dev, int64_t* n_app);
+/* Non-apparent columns in coboundary order. */
+int rips_nonapparent(rips_ctx* ctx, int d, const float** diam_dev, const uint64_t** cidx_dev, int64_t* n_non);
+/* All pivots of dimension d (apparent pairs united with the reduced ones), ascending by cidx(t).
+ * d = 0: t = merging edge, s = the vertex that gave birth to the dying component. */
+int rips_pivots(rips_ctx* ctx, int d, const uint64_t** t_dev, const uint64_t** s_dev, int64_t* n_piv);
+/* Two-layer pair store lookup: s_out_dev[i] = cidx(s) of the pivot whose row is
+ * t_query_dev[i], or -1.  Device binary search over the sorted arrays. */
+int rips_pivot_lookup(rips_ctx* ctx, int d, const uint64_t* t_query_dev, int64_t m, int64_t* s_out_dev);
+
+int rips_stats(rips_ctx* ctx, int d, rips_stats_t* out);
+int rips_timings(rips_ctx* ctx, int d, rips_timings_t* out);
+
+/* Device bytes currently held by the context. */
+int rips_device_bytes(rips_ctx* ctx, int64_t* bytes);
+/* Number of kernels this context has launched so far. */
+int rips_kernel_launches(rips_ctx* ctx, int64_t* launches);
+
+/* Standalone primitive, exposed for tests and benches: stable LSD onesweep radix sort of n 64-bit
+ * records on bits [lo_bit, hi_bit) (ascending), device pointers, tmp_dev = n more records.  The
+ * sorted data ends in keys_dev.  stream as in rips_init. */
+int rips_sort_u64(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, int hi_bit, void* stream);
+
+const char* rips_strerror(int code);
+/* Text of the last CUDA error seen by this thread's calls ("" if none). */
+const char* rips_last_error(void);
+void rips_free(rips_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RIPS_H */

@@ -1,0 +1,89 @@
+// kernels.cuh -- host-side launchers of the hot-path kernels (definitions in stage1.cu, stage2.cu,
+// dim0.cu, init.cu).  Packed records used throughout the device path:
+//
+//   column record   (key << cbits) | cidx      key = descending dense rank of the diameter
+//                                               (0 = largest distance), cbits = bits of C(n,d+1)-1
+//   pair record     (cidx(t) << 3) | j         j = position of the added vertex v inside t
+//                                               (number of vertices of s below v); s = t minus that vertex
+//
+// Both are bijective encodings of the paper's (diameter, cidx) struct and
+// (t, s) key-value pair; the fp32 / two-array forms the C ABI exposes are produced
+// from them by the unpack kernels.
+#pragma once
+#include "common.cuh"
+
+#define RIPS_MAX_M 6           // vertices of a column simplex: d+1 <= 6  (dim_max <= 4, scale row d = dim_max+1)
+#define RIPS_PAIR_POS_BITS 3
+
+// ------------------------------------------------------------------ init.cu
+// rec[e] = (~bits(dist[e]) << 32) | e ; dist canonicalised in place (-0 -> +0); *bad |= 1 on NaN / inf / negative
+cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, cudaStream_t st);
+// sorted rec (value descending, e ascending) -> K[e] = dense rank, values[rank]; *n_distinct
+cudaError_t launch_rank_edges(const u64* rec_sorted, i64 E, u32* K, float* values, u64* status, u32* ticket,
+                              u64* n_distinct, cudaStream_t st);
+i64 rank_edges_tiles(i64 E);
+
+// ------------------------------------------------------------------ dim0.cu
+struct Dim0Out {
+    u64* pair_ts;   // [n-1] packed (edge cidx << 16) | birth vertex of the dying component, in merge order
+    float* death;   // [n-1] diameter of the merging edge
+    u32* n_pairs;   // scalar
+};
+cudaError_t launch_dim0(const u64* rec_sorted, i64 E, int n, u32 thr_bits_inv, u32* parent_maxv /*2n*/, Dim0Out out,
+                        cudaStream_t st);
+
+// ------------------------------------------------------------------ stage1.cu
+struct ClearSet {
+    const u32* bitmap;     // bit idx set <=> idx is a pivot row of dimension d-1 (NULL: use the sorted arrays)
+    const u64* layer1;     // sorted packed pair records of dimension d-1 (t = rec >> shift1)
+    i64 n1;
+    int shift1;
+    const u64* layer2;     // sorted t of the reduced pivots
+    i64 n2;
+};
+struct Stage1Params {
+    const u32* K;
+    BinomTable bt;
+    int n;
+    u64 total;        // C(n, d+1)
+    u32 thr_key;      // keep iff key >= thr_key
+    int cbits;
+    ClearSet clear;
+    u64* out;         // packed column records in increasing cidx; NULL = count only
+    u64* status;      // one word per tile, zeroed
+    u32* ticket;      // zeroed
+    u64* counters;    // [0] kept [1] removed by diameter [2] cleared ; zeroed
+};
+i64 stage1_tiles(u64 total);
+cudaError_t launch_stage1(int M, const Stage1Params& p, cudaStream_t st);
+// bitmap |= bits of the given pivot rows
+cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, cudaStream_t st);
+
+// ------------------------------------------------------------------ stage2.cu
+struct Stage2Params {
+    const u64* cols;  // sorted packed column records
+    i64 len;
+    const u32* K;
+    BinomTable bt;
+    int n;
+    int cbits;
+    u64* app_out;     // packed pair records, in column order (sorted by t afterwards)
+    u64* non_out;     // packed column records of the non-apparent columns, in column order
+    u64* status_app;  // one word per tile each, zeroed
+    u64* status_non;
+    u32* ticket;      // zeroed
+    u64* counters;    // [0] apparent [1] non-apparent ; zeroed
+};
+i64 stage2_tiles(i64 len);
+cudaError_t launch_stage2(int M, const Stage2Params& p, cudaStream_t st);
+
+// ------------------------------------------------------------------ unpack / lookup (stage2.cu)
+cudaError_t launch_unpack_columns(const u64* cols, i64 len, int cbits, const float* values, float* diam, u64* cidx,
+                                  cudaStream_t st);
+// packed pair records -> t[], s[]   (M = vertices of s)
+cudaError_t launch_unpack_pairs(int M, const u64* pairs, i64 len, BinomTable bt, int n, u64* t, u64* s, cudaStream_t st);
+// merge of the two layers into one array ascending by t (layer 1 unpacked on the fly)
+cudaError_t launch_merge_pivots(int M, const u64* pairs, i64 n1, BinomTable bt, int n, const u64* red_t, const u64* red_s,
+                                i64 n2, u64* t, u64* s, cudaStream_t st);
+cudaError_t launch_pivot_lookup(int M, const u64* pairs, i64 n1, BinomTable bt, int n, const u64* red_t, const u64* red_s,
+                                i64 n2, const u64* query, i64 m, i64* s_out, cudaStream_t st);

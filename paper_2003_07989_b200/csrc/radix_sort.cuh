@@ -1,0 +1,32 @@
+// radix_sort.cuh -- interface of the hand-written onesweep radix sort (no CUB, no Thrust).
+// Step a6 / a9 of DESIGN.md: the paper's "GPU-sort" (pair array sorted by
+// row).
+#pragma once
+#include "common.cuh"
+
+#define RIPS_SORT_MAX_PASSES 8
+#define RIPS_SORT_MAX_BINS 512
+
+struct SortPlan {
+    int npasses;
+    int shift[RIPS_SORT_MAX_PASSES];
+    int bits[RIPS_SORT_MAX_PASSES];
+    i64 tile_items;
+};
+
+// Digits covering bits [lo_bit, hi_bit): as few passes as 9-bit digits allow, widths balanced.
+SortPlan sort_make_plan(int lo_bit, int hi_bit);
+
+// Scratch the sort needs besides the ping-pong buffer, in bytes (status words, histograms, ticket).
+size_t sort_scratch_bytes(i64 n, const SortPlan& plan);
+
+struct SortTimes {
+    cudaEvent_t ev[3]; // optional: [0] before histogram, [1] after histogram, [2] after the last pass
+    bool enabled;
+};
+
+// Stable LSD sort of n u64 records by the plan's digits, ascending.  `a` holds the input, `b` is the
+// ping-pong buffer; returns (via *result) which of the two holds the sorted data (a if the number
+// of passes is even).  scratch: sort_scratch_bytes(n, plan) device bytes.  launches += kernels run.
+cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
+                     u64** result, SortTimes* times, i64* launches);
