@@ -1,0 +1,52 @@
+"""Build the C-ABI shared library `librips_b200.so` in-tree with nvcc for sm_100a.
+
+    python -m paper_2003_07989_b200.build [--force] [--verbose]
+
+The sources are csrc/*.cu (hand-written CUDA) and csrc/reduce_host.cpp; the only public header is
+include/rips.h.  The .so is git-ignored but travels to the GPU box with the tree.
+"""
+from __future__ import annotations
+
+import os
+import shutil
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "librips_b200.so")
+SOURCES = ["rips.cu", "radix_sort.cu", "stage1.cu", "stage2.cu", "dim0.cu", "init.cu", "reduce_host.cpp"]
+HEADERS = ["common.cuh", "kernels.cuh", "radix_sort.cuh", "reduce_host.h", os.path.join("..", "..", "include", "rips.h")]
+
+
+def nvcc() -> str:
+    exe = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(exe):
+        raise RuntimeError("nvcc not found: the CUDA path cannot be built (there is no CPU fallback)")
+    return exe
+
+
+def needs_build() -> bool:
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and not needs_build():
+        return LIB
+    tmp = LIB + f".{os.getpid()}.tmp"
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+           "-shared", "-Xcompiler", "-fPIC,-O3", "--use_fast_math" if False else "-Xcompiler", "-Wall",
+           "-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
+    if verbose:
+        cmd.insert(1, "-Xptxas")
+        cmd.insert(2, "-v")
+    subprocess.check_call(cmd)
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

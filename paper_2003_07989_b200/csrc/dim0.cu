@@ -1,0 +1,108 @@
+// dim0.cu -- dimension 0 on the GPU (union-find over the edges in filtration order;
+// the paper keeps it on the CPU).  Not the hot path; timed separately.
+// Filter-Kruskal in one CTA: the sorted edge records of rips_init (value descending, cidx
+// ascending) read backwards ARE the filtration order of the 1-simplices (diameter ascending,
+// cidx descending).  Each round 1024 threads test 1024 edges against the current
+// forest in parallel (read-mostly finds with path compression); the few edges whose endpoints are
+// still in different components are compacted in order and merged serially by one thread, which
+// is what makes the result independent of scheduling.  The loop stops after n-1 merges.
+#include "kernels.cuh"
+
+namespace {
+
+constexpr int D0_THREADS = 1024;
+
+__device__ __forceinline__ void edge_vertices(u32 e, int* a, int* b)
+{
+    int i = (int)((1.0 + sqrt(1.0 + 8.0 * (double)e)) * 0.5);
+    while ((u64)i * (u64)(i - 1) / 2 > (u64)e) --i;
+    while ((u64)(i + 1) * (u64)i / 2 <= (u64)e) ++i;
+    *a = i;
+    *b = (int)(e - (u32)((u64)i * (u64)(i - 1) / 2));
+}
+
+__device__ __forceinline__ u32 find_root(volatile u32* parent, u32 x)
+{
+    u32 r = x;
+    while (parent[r] != r) r = parent[r];
+    // compression: every write stores an ancestor, so concurrent readers always see a valid forest
+    while (parent[x] != r) { u32 nx = parent[x]; parent[x] = r; x = nx; }
+    return r;
+}
+
+__global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict__ rec, i64 E, int n, u32 thr_inv,
+                                                          u32* parent_maxv, Dim0Out out)
+{
+    __shared__ u32 s_list[D0_THREADS];
+    __shared__ u32 s_wcount[D0_THREADS / 32];
+    __shared__ i64 s_start;
+    __shared__ u32 s_merges;
+    volatile u32* parent = parent_maxv;
+    volatile u32* maxv = parent_maxv + n;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < n; i += D0_THREADS) { parent[i] = i; maxv[i] = i; }
+    if (tid == 0) {
+        // first position whose value is <= threshold (records are value-descending = inverted bits ascending)
+        i64 lo = 0, hi = E;
+        while (lo < hi) {
+            i64 mid = lo + ((hi - lo) >> 1);
+            if ((u32)(rec[mid] >> 32) < thr_inv) lo = mid + 1;
+            else hi = mid;
+        }
+        s_start = lo;
+        s_merges = 0;
+    }
+    __syncthreads();
+    const i64 start = s_start;
+    for (i64 hi = E; hi > start; hi -= D0_THREADS) {
+        const i64 i = hi - 1 - tid;
+        bool cand = false;
+        if (i >= start) {
+            int a, b;
+            edge_vertices((u32)rec[i], &a, &b);
+            cand = find_root(parent, a) != find_root(parent, b);
+        }
+        const u32 bal = __ballot_sync(RIPS_FULL_MASK, cand);
+        if (lane == 0) s_wcount[warp] = __popc(bal);
+        __syncthreads();
+        u32 off = 0, tot = 0;
+        for (int w = 0; w < D0_THREADS / 32; ++w) {
+            u32 c = s_wcount[w];
+            if (w < warp) off += c;
+            tot += c;
+        }
+        if (cand) s_list[off + __popc(bal & ((1u << lane) - 1u))] = (u32)(hi - 1 - i); // = tid, kept for clarity
+        __syncthreads();
+        if (tid == 0) {
+            u32 m = s_merges;
+            for (u32 c = 0; c < tot && m < (u32)(n - 1); ++c) {
+                const u64 r = rec[hi - 1 - s_list[c]];
+                int a, b;
+                edge_vertices((u32)r, &a, &b);
+                u32 ra = find_root(parent, a), rb = find_root(parent, b);
+                if (ra == rb) continue;
+                // a component is born with its largest vertex (vertices enter in decreasing index,
+                // PAPER.md:79); the younger component, the one with the smaller largest vertex, dies
+                u32 dying = (maxv[ra] < maxv[rb]) ? ra : rb;
+                u32 living = (dying == ra) ? rb : ra;
+                out.pair_ts[m] = ((u64)(u32)r << 16) | (u64)maxv[dying];
+                out.death[m] = __uint_as_float(~(u32)(r >> 32));
+                parent[dying] = living;
+                ++m;
+            }
+            s_merges = m;
+        }
+        __syncthreads();
+        if (s_merges >= (u32)(n - 1)) break;
+    }
+    if (tid == 0) *out.n_pairs = s_merges;
+}
+
+} // namespace
+
+cudaError_t launch_dim0(const u64* rec_sorted, i64 E, int n, u32 thr_bits_inv, u32* parent_maxv, Dim0Out out,
+                        cudaStream_t st)
+{
+    dim0_kernel<<<1, D0_THREADS, 0, st>>>(rec_sorted, E, n, thr_bits_inv, parent_maxv, out);
+    return cudaGetLastError();
+}

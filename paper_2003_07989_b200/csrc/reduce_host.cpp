@@ -1,0 +1,146 @@
+// reduce_host.cpp -- see reduce_host.h.  Implicit cohomology reduction over Z/2 (PAPER.md:127,
+// :168-170, :210) of the columns stage 2 left, with the two-layer pair store of PAPER.md:555-561:
+// pivots found here go to a hash map, apparent pairs are looked up by binary search in the sorted
+// array.  Column entries are packed (key << tbits) | cidx(t); the pivot of a column is the cofacet
+// that comes first in the filtration order (smallest diameter = LARGEST key, then largest cidx,
+// PAPER.md:77-79), i.e. simply the largest packed entry.
+#include "reduce_host.h"
+
+#include <queue>
+#include <unordered_map>
+
+namespace {
+
+struct Ctx {
+    const HostReduceIn& in;
+    int M; // vertices of a column simplex
+    explicit Ctx(const HostReduceIn& i) : in(i), M(i.d + 1) {}
+    uint64_t C(int v, int k) const { return in.binom[(size_t)k * in.bstride + v]; }
+    uint32_t key(int a, int b) const
+    {
+        int hi = a > b ? a : b, lo = a > b ? b : a;
+        return in.K[(size_t)hi * (hi - 1) / 2 + lo];
+    }
+    void decode(uint64_t idx, int m, int* v) const
+    { // v[m-1] > ... > v[0]
+        int hi = in.n - 1;
+        for (int k = m; k >= 1; --k) {
+            int lo = k - 1, h = hi;
+            while (lo < h) {
+                int mid = (lo + h + 1) >> 1;
+                if (C(mid, k) <= idx) lo = mid;
+                else h = mid - 1;
+            }
+            v[k - 1] = lo;
+            idx -= C(lo, k);
+            hi = lo - 1;
+        }
+    }
+    // first-layer lookup: s of the apparent pair whose row is t, or false
+    bool apparent_lookup(uint64_t t, uint64_t* s) const
+    {
+        int64_t lo = 0, hi = in.n_app;
+        while (lo < hi) {
+            int64_t mid = lo + (hi - lo) / 2;
+            if ((in.app[mid] >> 3) < t) lo = mid + 1;
+            else hi = mid;
+        }
+        if (lo >= in.n_app || (in.app[lo] >> 3) != t) return false;
+        int j = (int)(in.app[lo] & 7u), tv[16];
+        decode(t, M + 1, tv);
+        uint64_t r = 0;
+        for (int i = 0; i <= M; ++i) {
+            if (i < j) r += C(tv[i], i + 1);
+            else if (i > j) r += C(tv[i], i);
+        }
+        *s = r;
+        return true;
+    }
+    // push the coboundary of the column simplex s (cofacets with diameter <= threshold)
+    template <class Heap>
+    uint32_t push_coboundary(Heap& h, uint64_t cidx_s) const
+    {
+        int s[16];
+        decode(cidx_s, M, s);
+        uint32_t key_s = 0xffffffffu;
+        for (int a = 1; a < M; ++a)
+            for (int b = 0; b < a; ++b) { uint32_t k = key(s[a], s[b]); if (k < key_s) key_s = k; }
+        uint64_t low[17], high[17]; // low[g] = sum_{i<g} C(s[i], i+1); high[g] = sum_{i>=g} C(s[i], i+2)
+        low[0] = 0;
+        for (int i = 0; i < M; ++i) low[i + 1] = low[i] + C(s[i], i + 1);
+        high[M] = 0;
+        for (int i = M - 1; i >= 0; --i) high[i] = high[i + 1] + C(s[i], i + 2);
+        for (int seg = M; seg >= 0; --seg) {
+            int hi = (seg == M) ? in.n - 1 : s[seg] - 1;
+            int lo = (seg == 0) ? 0 : s[seg - 1] + 1;
+            for (int v = hi; v >= lo; --v) {
+                uint32_t kt = key_s;
+                for (int j = 0; j < M; ++j) { uint32_t k = key(v, s[j]); if (k < kt) kt = k; }
+                if (kt < in.thr_key) continue;
+                uint64_t t = low[seg] + C(v, seg + 1) + high[seg];
+                h.push(((uint64_t)kt << in.tbits) | t);
+            }
+        }
+        return key_s;
+    }
+};
+
+template <class Heap>
+bool pop_pivot(Heap& h, uint64_t* piv)
+{
+    while (!h.empty()) {
+        uint64_t p = h.top();
+        h.pop();
+        if (!h.empty() && h.top() == p) { h.pop(); continue; } // equal entries cancel over Z/2
+        *piv = p;
+        return true;
+    }
+    return false;
+}
+
+} // namespace
+
+void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
+{
+    Ctx cx(in);
+    const uint64_t cmask = (in.cbits >= 64) ? ~0ull : ((1ull << in.cbits) - 1ull);
+    const uint64_t tmask = (1ull << in.tbits) - 1ull;
+    std::unordered_map<uint64_t, uint64_t> found; // second layer: t -> s for pivots found here
+    found.reserve((size_t)in.ncols * 2 + 16);
+    std::vector<uint64_t> store;
+    for (int64_t j = 0; j < in.ncols; ++j) {
+        const uint64_t cidx_s = in.cols[j] & cmask;
+        const uint32_t key_s = (uint32_t)(in.cols[j] >> in.cbits);
+        store.clear();
+        std::priority_queue<uint64_t, std::vector<uint64_t>> h(std::less<uint64_t>(), std::move(store));
+        cx.push_coboundary(h, cidx_s);
+        for (;;) {
+            uint64_t piv;
+            if (!pop_pivot(h, &piv)) {
+                out.ess_s.push_back(cidx_s);
+                out.ess_key.push_back(key_s);
+                out.ess_col.push_back(j);
+                break;
+            }
+            const uint64_t t = piv & tmask;
+            uint64_t s2 = 0;
+            bool hit = false;
+            ++out.lookups;
+            auto it = found.find(t);
+            if (it != found.end()) { hit = true; s2 = it->second; }
+            else hit = cx.apparent_lookup(t, &s2);
+            if (!hit) {
+                found.emplace(t, cidx_s);
+                out.piv_t.push_back(t);
+                out.piv_s.push_back(cidx_s);
+                out.piv_key_t.push_back((uint32_t)(piv >> in.tbits));
+                out.piv_key_s.push_back(key_s);
+                out.piv_col.push_back(j);
+                break;
+            }
+            h.push(piv); // the column of s2 contains t as well: the two cancel
+            cx.push_coboundary(h, s2);
+            ++out.additions;
+        }
+    }
+}

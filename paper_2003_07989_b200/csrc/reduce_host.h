@@ -1,0 +1,32 @@
+// reduce_host.h -- the serial remainder: reduction of the non-apparent columns (Algorithm 2,
+// PAPER.md:182-200; "submatrix reduction").  NOT the hot path: it runs on the
+// host, as in the paper, and is timed and reported separately (rips_timings).
+#pragma once
+#include <stdint.h>
+#include <vector>
+
+struct HostReduceIn {
+    int n, d;
+    const uint32_t* K;        // host copy of the key matrix (lower triangle)
+    const uint64_t* binom;    // host binomial table, k-major, stride n+1
+    int bstride;
+    uint32_t thr_key;         // cofacets with key < thr_key are above the threshold
+    const uint64_t* cols;     // packed column records of the non-apparent columns, coboundary order
+    int64_t ncols;
+    int cbits;
+    const uint64_t* app;      // packed pair records ascending by t (first layer of the pair store)
+    int64_t n_app;
+    int tbits;                // bits of C(n, d+2) - 1
+};
+
+struct HostReduceOut {
+    std::vector<uint64_t> piv_t, piv_s; // pivots found, in processing order
+    std::vector<uint32_t> piv_key_t, piv_key_s;
+    std::vector<uint64_t> ess_s;        // zero columns
+    std::vector<uint32_t> ess_key;
+    std::vector<int64_t> piv_col, ess_col; // position of the column in `cols`
+    int64_t additions = 0;
+    int64_t lookups = 0;
+};
+
+void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out);

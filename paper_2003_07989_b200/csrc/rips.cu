@@ -1,0 +1,868 @@
+// rips.cu -- context, per-dimension driver and the C ABI of include/rips.h.
+// Control flow (Fig. 3(b)): dim 0, then per d: stage 1 (clear bitmap ->
+// enumerate/filter/compact -> onesweep sort), stage 2 (apparent kernel with partition -> pair sort),
+// reduction of the few non-apparent columns (host, not hot path), next d.
+#include "../../include/rips.h"
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+#include "radix_sort.cuh"
+#include "reduce_host.h"
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int cuda_fail(cudaError_t e, const char* what)
+{
+    g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return RIPS_ECUDA;
+}
+#define CU(x)                                        \
+    do {                                             \
+        cudaError_t e__ = (x);                       \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #x); \
+    } while (0)
+#define RC(x)                  \
+    do {                       \
+        int r__ = (x);         \
+        if (r__ != RIPS_OK) return r__; \
+    } while (0)
+
+// A device buffer that is reused while large enough.
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+};
+
+enum Ev {
+    EV_S1_BEGIN, EV_S1_BITMAP, EV_S1_ENUM, EV_S1_SORTBEG, EV_S1_HIST, EV_S1_SORT, EV_S1_END,
+    EV_S2_BEGIN, EV_S2_APP, EV_S2_SORTBEG, EV_S2_HIST, EV_S2_SORT, EV_S2_END,
+    EV_D0_BEGIN, EV_D0_END, EV_COUNT
+};
+
+struct DimState {
+    // sizes
+    u64 total = 0;   // C(n, d+1)
+    int M = 0;       // d + 1
+    int cbits = 0, tbits = 0;
+    // stage 1
+    bool have_s1 = false;
+    DevBuf colsA, colsB, s1_status, bitmap;
+    u64* cols = nullptr; // sorted packed column records (points into colsA or colsB)
+    i64 len = 0;
+    // stage 2
+    bool have_s2 = false;
+    DevBuf appA, appB, non, s2_status;
+    u64* app = nullptr; // sorted packed pair records
+    i64 n_app = 0, n_non = 0;
+    // reduction (second layer), sorted by t
+    bool have_red = false;
+    DevBuf red_t, red_s;
+    i64 n_red = 0;
+    // lazily materialised views
+    DevBuf v_fdiam, v_fcidx, v_at, v_as, v_ndiam, v_ncidx, v_pt, v_ps;
+    bool has_vf = false, has_va = false, has_vn = false, has_vp = false;
+    std::vector<float> bars;
+    rips_stats_t stats;
+    rips_timings_t tim;
+    cudaEvent_t ev[EV_COUNT];
+    bool ev_rec[EV_COUNT];
+    bool ev_made = false;
+};
+
+} // namespace
+
+struct rips_ctx {
+    i64 n = 0, E = 0;
+    int dim_max = 0;
+    float threshold = 0;
+    cudaStream_t stream = 0;
+    int kmax = 0; // binomial table holds C(v,k), k <= kmax
+    std::vector<u64> h_binom;
+    std::vector<float> h_values;
+    std::vector<u32> h_K; // host copy of the key matrix, made on first use by the reduction
+    float* d_dist = nullptr;
+    u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
+    u32* d_K = nullptr;
+    float* d_values = nullptr;
+    u64* d_binom = nullptr;
+    u64* d_counters = nullptr; // 8 u64 scratch counters
+    u32* d_tickets = nullptr;  // 8 u32
+    u64* h_counters = nullptr; // pinned
+    u32 n_distinct = 0, thr_key = 0;
+    int key_bits = 1;
+    DevBuf sort_scratch;
+    // dim 0
+    DevBuf d0_pairs, d0_death, d0_uf;
+    std::vector<DimState> dims; // index d, 0 .. dim_max+1
+    i64 dev_bytes = 0, launches = 0;
+    BinomTable bt() const { return BinomTable{d_binom, (int)(n + 1)}; }
+};
+
+namespace {
+
+int ensure(rips_ctx* c, DevBuf& b, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    if (b.cap >= bytes) return RIPS_OK;
+    if (b.p) { cudaFree(b.p); c->dev_bytes -= (i64)b.cap; b.p = nullptr; b.cap = 0; }
+    cudaError_t e = cudaMalloc(&b.p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        g_last_error = "cudaMalloc of " + std::to_string(bytes) + " bytes failed: " + cudaGetErrorString(e);
+        b.p = nullptr;
+        return e == cudaErrorMemoryAllocation ? RIPS_ENOMEM : RIPS_ECUDA;
+    }
+    b.cap = bytes;
+    c->dev_bytes += (i64)bytes;
+    return RIPS_OK;
+}
+void release(rips_ctx* c, DevBuf& b)
+{
+    if (b.p) { cudaFree(b.p); c->dev_bytes -= (i64)b.cap; }
+    b.p = nullptr;
+    b.cap = 0;
+}
+
+void ev_record(rips_ctx* c, DimState& s, int which)
+{
+    if (!s.ev_made) {
+        for (int i = 0; i < EV_COUNT; ++i) { cudaEventCreate(&s.ev[i]); s.ev_rec[i] = false; }
+        s.ev_made = true;
+    }
+    cudaEventRecord(s.ev[which], c->stream);
+    s.ev_rec[which] = true;
+}
+float ev_ms(DimState& s, int a, int b)
+{
+    if (!s.ev_made || !s.ev_rec[a] || !s.ev_rec[b]) return 0.f;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, s.ev[a], s.ev[b]) != cudaSuccess) { cudaGetLastError(); return 0.f; }
+    return ms;
+}
+
+// saturating binomial table, k-major
+bool build_binom(i64 n, int kmax, std::vector<u64>& out)
+{
+    const size_t stride = (size_t)n + 1;
+    out.assign((size_t)(kmax + 1) * stride, 0);
+    for (size_t v = 0; v <= (size_t)n; ++v) out[v] = 1; // C(v,0)
+    for (int k = 1; k <= kmax; ++k)
+        for (size_t v = 1; v <= (size_t)n; ++v) {
+            u64 a = out[(size_t)(k - 1) * stride + v - 1], b = out[(size_t)k * stride + v - 1];
+            out[(size_t)k * stride + v] = (a > ~0ull - b) ? ~0ull : a + b;
+        }
+    return true;
+}
+u64 hbinom(const rips_ctx* c, i64 v, int k)
+{
+    if (k < 0 || v < 0 || k > c->kmax) return 0;
+    return c->h_binom[(size_t)k * (c->n + 1) + v];
+}
+
+void invalidate_views(DimState& s, bool f, bool a, bool nn, bool p)
+{
+    if (f) s.has_vf = false;
+    if (a) s.has_va = false;
+    if (nn) s.has_vn = false;
+    if (p) s.has_vp = false;
+}
+
+double now_ms()
+{
+    using namespace std::chrono;
+    return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
+}
+
+// ------------------------------------------------------------------------------------------ dim 0
+int run_dim0(rips_ctx* c)
+{
+    DimState& s = c->dims[0];
+    const i64 n = c->n;
+    s.M = 1;
+    s.total = (u64)n;
+    s.stats = rips_stats_t{};
+    s.stats.n_candidates = n;
+    s.bars.clear();
+    RC(ensure(c, c->d0_pairs, (size_t)n * 8));
+    RC(ensure(c, c->d0_death, (size_t)n * 4));
+    RC(ensure(c, c->d0_uf, (size_t)n * 8));
+    i64 npairs = 0;
+    ev_record(c, s, EV_D0_BEGIN);
+    if (n >= 2 && c->threshold >= 0.0f) {
+        u32 thr_bits;
+        float thr = c->threshold;
+        memcpy(&thr_bits, &thr, 4);
+        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+        Dim0Out out{(u64*)c->d0_pairs.p, (float*)c->d0_death.p, (u32*)c->d_counters};
+        CU(launch_dim0(c->d_edges, c->E, (int)n, ~thr_bits, (u32*)c->d0_uf.p, out, c->stream));
+        c->launches += 1;
+        ev_record(c, s, EV_D0_END);
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        npairs = (i64)(u32)c->h_counters[0];
+    } else {
+        ev_record(c, s, EV_D0_END);
+    }
+    // n-1 items at most: order them by edge index on the host, upload as the (only) pivot layer
+    std::vector<u64> ts((size_t)npairs);
+    std::vector<float> death((size_t)npairs);
+    if (npairs) {
+        CU(cudaMemcpy(ts.data(), c->d0_pairs.p, (size_t)npairs * 8, cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(death.data(), c->d0_death.p, (size_t)npairs * 4, cudaMemcpyDeviceToHost));
+    }
+    std::vector<i64> order((size_t)npairs);
+    for (i64 i = 0; i < npairs; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](i64 a, i64 b) { return ts[a] < ts[b]; });
+    std::vector<u64> t((size_t)npairs), sv((size_t)npairs);
+    for (i64 i = 0; i < npairs; ++i) {
+        u64 r = ts[order[i]];
+        t[i] = r >> 16;
+        sv[i] = r & 0xffffu;
+        float dd = death[order[i]];
+        if (dd > 0.0f) { s.bars.push_back(0.0f); s.bars.push_back(dd); }
+    }
+    for (i64 i = 0; i < n - npairs; ++i) { s.bars.push_back(0.0f); s.bars.push_back(INFINITY); }
+    RC(ensure(c, s.red_t, (size_t)npairs * 8));
+    RC(ensure(c, s.red_s, (size_t)npairs * 8));
+    if (npairs) {
+        CU(cudaMemcpy(s.red_t.p, t.data(), (size_t)npairs * 8, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(s.red_s.p, sv.data(), (size_t)npairs * 8, cudaMemcpyHostToDevice));
+    }
+    s.n_red = npairs;
+    s.n_app = 0;
+    s.app = nullptr;
+    s.have_s1 = s.have_s2 = s.have_red = true;
+    s.stats.n_columns = n;
+    s.stats.n_reduced_pivots = npairs;
+    s.stats.n_essential = n - npairs;
+    s.stats.n_bars = (i64)s.bars.size() / 2;
+    invalidate_views(s, true, true, true, true);
+    return RIPS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ stage 1
+int run_stage1(rips_ctx* c, int d)
+{
+    if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    DimState& prev = c->dims[d - 1];
+    if (!prev.have_red) { g_last_error = "rips_stage1: pivots of the previous dimension are missing"; return RIPS_EINVAL; }
+    const i64 n = c->n;
+    s.M = d + 1;
+    s.total = hbinom(c, n, d + 1);
+    s.cbits = bits_for(s.total ? s.total - 1 : 0);
+    if (c->key_bits + s.cbits > 64) return RIPS_EOVERFLOW;
+    s.have_s1 = s.have_s2 = s.have_red = false;
+    invalidate_views(s, true, true, true, true);
+    rips_stats_t keep_stats = rips_stats_t{};
+    s.stats = keep_stats;
+    s.stats.n_candidates = (i64)s.total;
+    s.stats.key_bits = c->key_bits;
+    s.stats.index_bits = s.cbits;
+    s.len = 0;
+    s.cols = nullptr;
+    ev_record(c, s, EV_S1_BEGIN);
+    if (s.total == 0) {
+        ev_record(c, s, EV_S1_BITMAP); ev_record(c, s, EV_S1_ENUM); ev_record(c, s, EV_S1_SORTBEG);
+        ev_record(c, s, EV_S1_HIST); ev_record(c, s, EV_S1_SORT); ev_record(c, s, EV_S1_END);
+        s.have_s1 = true;
+        return RIPS_OK;
+    }
+    // ---- a4: clearing set of dimension d-1 as a bitmap over the candidate indices
+    const u64 words = (s.total + 31) / 32;
+    const bool use_bitmap = words * 4 <= (8ull << 30);
+    ClearSet cs{nullptr, prev.app, prev.n_app, RIPS_PAIR_POS_BITS, (const u64*)prev.red_t.p, prev.n_red};
+    if (use_bitmap) {
+        RC(ensure(c, s.bitmap, (size_t)words * 4));
+        CU(cudaMemsetAsync(s.bitmap.p, 0, (size_t)words * 4, c->stream));
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.app, prev.n_app, RIPS_PAIR_POS_BITS, c->stream));
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, 0, c->stream));
+        c->launches += (prev.n_app > 0) + (prev.n_red > 0);
+        cs.bitmap = (const u32*)s.bitmap.p;
+    }
+    ev_record(c, s, EV_S1_BITMAP);
+    // ---- a3-a5
+    const i64 tiles = stage1_tiles(s.total);
+    RC(ensure(c, s.s1_status, (size_t)tiles * 8));
+    Stage1Params p;
+    p.K = c->d_K;
+    p.bt = c->bt();
+    p.n = (int)n;
+    p.total = s.total;
+    p.thr_key = c->thr_key;
+    p.cbits = s.cbits;
+    p.clear = cs;
+    p.status = (u64*)s.s1_status.p;
+    p.ticket = c->d_tickets;
+    p.counters = c->d_counters;
+    u64 cap;
+    if (c->thr_key == 0) {
+        cap = s.total - (u64)(prev.n_app + prev.n_red); // every pivot row of d-1 is a candidate below the threshold
+    } else {
+        size_t free_b = 0, total_b = 0;
+        cudaMemGetInfo(&free_b, &total_b);
+        cap = s.total;
+        if (s.total * 8 > free_b / 8 && s.colsA.cap < s.total * 8) { // count first, then allocate exactly
+            CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+            CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+            p.out = nullptr;
+            CU(launch_stage1(s.M, p, c->stream));
+            c->launches += 1;
+            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            cap = c->h_counters[0];
+        }
+    }
+    RC(ensure(c, s.colsA, (size_t)cap * 8));
+    CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+    CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+    CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
+    p.out = (u64*)s.colsA.p;
+    CU(launch_stage1(s.M, p, c->stream));
+    c->launches += 1;
+    ev_record(c, s, EV_S1_ENUM);
+    CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    s.len = (i64)c->h_counters[0];
+    s.stats.n_columns = s.len;
+    s.stats.n_removed_by_diameter = (i64)c->h_counters[1];
+    s.stats.n_cleared = (i64)c->h_counters[2];
+    // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys
+    SortPlan plan = sort_make_plan(s.cbits, s.cbits + c->key_bits);
+    s.stats.sort_passes = s.len > 1 ? plan.npasses : 0;
+    RC(ensure(c, s.colsB, (size_t)s.len * 8));
+    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.len, plan)));
+    SortTimes st;
+    st.enabled = true;
+    if (!s.ev_made) ev_record(c, s, EV_S1_SORTBEG);
+    st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
+    s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
+    u64* res = nullptr;
+    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
+    s.cols = res;
+    ev_record(c, s, EV_S1_END);
+    s.have_s1 = true;
+    return RIPS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ stage 2
+int run_stage2(rips_ctx* c, int d)
+{
+    if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s1) { g_last_error = "rips_stage2: rips_stage1 has not run for this dimension"; return RIPS_EINVAL; }
+    const i64 n = c->n;
+    const u64 rows = hbinom(c, n, d + 2);
+    if (rows == ~0ull) return RIPS_EOVERFLOW;
+    s.tbits = bits_for(rows ? rows - 1 : 0);
+    if (s.tbits + RIPS_PAIR_POS_BITS > 64 || s.tbits + c->key_bits > 64) return RIPS_EOVERFLOW;
+    s.have_s2 = s.have_red = false;
+    invalidate_views(s, false, true, true, true);
+    s.n_app = s.n_non = 0;
+    s.app = nullptr;
+    ev_record(c, s, EV_S2_BEGIN);
+    const i64 tiles = stage2_tiles(s.len);
+    if (s.len > 0) {
+        RC(ensure(c, s.appA, (size_t)s.len * 8));
+        RC(ensure(c, s.non, (size_t)s.len * 8));
+        RC(ensure(c, s.s2_status, (size_t)tiles * 16));
+        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+        CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+        CU(cudaMemsetAsync(s.s2_status.p, 0, (size_t)tiles * 16, c->stream));
+        Stage2Params p;
+        p.cols = s.cols;
+        p.len = s.len;
+        p.K = c->d_K;
+        p.bt = c->bt();
+        p.n = (int)n;
+        p.cbits = s.cbits;
+        p.app_out = (u64*)s.appA.p;
+        p.non_out = (u64*)s.non.p;
+        p.status_app = (u64*)s.s2_status.p;
+        p.status_non = (u64*)s.s2_status.p + tiles;
+        p.ticket = c->d_tickets;
+        p.counters = c->d_counters;
+        CU(launch_stage2(s.M, p, c->stream));
+        c->launches += 1;
+    }
+    ev_record(c, s, EV_S2_APP);
+    if (s.len > 0) {
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        s.n_app = (i64)c->h_counters[0];
+        s.n_non = (i64)c->h_counters[1];
+    }
+    s.stats.n_apparent = s.n_app;
+    s.stats.n_nonapparent = s.n_non;
+    // ---- a9: pairs ascending by row index t
+    SortPlan plan = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
+    s.stats.pair_sort_passes = s.n_app > 1 ? plan.npasses : 0;
+    RC(ensure(c, s.appA, 16));
+    RC(ensure(c, s.appB, (size_t)s.n_app * 8));
+    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_app, plan)));
+    SortTimes st;
+    st.enabled = true;
+    st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
+    s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
+    u64* res = nullptr;
+    CU(sort_u64((u64*)s.appA.p, (u64*)s.appB.p, s.n_app, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
+    s.app = res;
+    ev_record(c, s, EV_S2_END);
+    s.have_s2 = true;
+    return RIPS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ reduction (not hot path)
+int run_reduce(rips_ctx* c, int d)
+{
+    if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s2) { g_last_error = "rips_reduce: rips_stage2 has not run for this dimension"; return RIPS_EINVAL; }
+    s.have_red = false;
+    invalidate_views(s, false, false, false, true);
+    s.bars.clear();
+    s.tim.reduce_host_ms = s.tim.reduce_xfer_ms = 0.f;
+    HostReduceOut out;
+    if (s.n_non > 0) {
+        double t0 = now_ms();
+        CU(cudaStreamSynchronize(c->stream));
+        if (c->h_K.empty() && c->E) {
+            c->h_K.resize((size_t)c->E);
+            CU(cudaMemcpy(c->h_K.data(), c->d_K, (size_t)c->E * 4, cudaMemcpyDeviceToHost));
+        }
+        std::vector<u64> h_non((size_t)s.n_non), h_app((size_t)s.n_app);
+        CU(cudaMemcpy(h_non.data(), s.non.p, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost));
+        if (s.n_app) CU(cudaMemcpy(h_app.data(), s.app, (size_t)s.n_app * 8, cudaMemcpyDeviceToHost));
+        double t1 = now_ms();
+        HostReduceIn in;
+        in.n = (int)c->n;
+        in.d = d;
+        in.K = c->h_K.data();
+        in.binom = c->h_binom.data();
+        in.bstride = (int)(c->n + 1);
+        in.thr_key = c->thr_key;
+        in.cols = h_non.data();
+        in.ncols = s.n_non;
+        in.cbits = s.cbits;
+        in.app = h_app.data();
+        in.n_app = s.n_app;
+        in.tbits = s.tbits;
+        host_reduce_columns(in, out);
+        double t2 = now_ms();
+        s.tim.reduce_host_ms = (float)(t2 - t1);
+        s.tim.reduce_xfer_ms = (float)(t1 - t0);
+    }
+    // bars in column order of the birth simplex: merge the two lists by column position
+    {
+        size_t a = 0, b = 0;
+        while (a < out.piv_col.size() || b < out.ess_col.size()) {
+            bool take_piv = b >= out.ess_col.size() || (a < out.piv_col.size() && out.piv_col[a] < out.ess_col[b]);
+            if (take_piv) {
+                if (out.piv_key_s[a] != out.piv_key_t[a]) {
+                    s.bars.push_back(c->h_values[out.piv_key_s[a]]);
+                    s.bars.push_back(c->h_values[out.piv_key_t[a]]);
+                }
+                ++a;
+            } else {
+                s.bars.push_back(c->h_values[out.ess_key[b]]);
+                s.bars.push_back(INFINITY);
+                ++b;
+            }
+        }
+    }
+    // second layer of the pair store, ascending by t
+    const i64 nr = (i64)out.piv_t.size();
+    std::vector<i64> order((size_t)nr);
+    for (i64 i = 0; i < nr; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](i64 x, i64 y) { return out.piv_t[x] < out.piv_t[y]; });
+    std::vector<u64> t((size_t)nr), sv((size_t)nr);
+    for (i64 i = 0; i < nr; ++i) { t[i] = out.piv_t[order[i]]; sv[i] = out.piv_s[order[i]]; }
+    double t3 = now_ms();
+    RC(ensure(c, s.red_t, (size_t)nr * 8));
+    RC(ensure(c, s.red_s, (size_t)nr * 8));
+    if (nr) {
+        CU(cudaMemcpy(s.red_t.p, t.data(), (size_t)nr * 8, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(s.red_s.p, sv.data(), (size_t)nr * 8, cudaMemcpyHostToDevice));
+    }
+    s.tim.reduce_xfer_ms += (float)(now_ms() - t3);
+    s.n_red = nr;
+    s.stats.n_reduced_pivots = nr;
+    s.stats.n_essential = (i64)out.ess_s.size();
+    s.stats.n_additions = out.additions;
+    s.stats.n_bars = (i64)s.bars.size() / 2;
+    s.have_red = true;
+    return RIPS_OK;
+}
+
+int check_dim(rips_ctx* c, int d, int lo)
+{
+    if (!c) return RIPS_EINVAL;
+    if (d < lo || d > c->dim_max + 1) return RIPS_EINVAL;
+    return RIPS_OK;
+}
+
+void free_dim(rips_ctx* c, DimState& s)
+{
+    DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.appA, &s.appB, &s.non, &s.s2_status, &s.red_t,
+                     &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
+    for (DevBuf* b : all) release(c, *b);
+    if (s.ev_made) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(s.ev[i]);
+    s.ev_made = false;
+}
+
+int init_device_tables(rips_ctx* c, const float* dist_lower)
+{
+    const i64 E = c->E, n = c->n;
+    CU(cudaMalloc(&c->d_counters, 64));
+    CU(cudaMalloc(&c->d_tickets, 32));
+    CU(cudaMallocHost(&c->h_counters, 64));
+    CU(cudaMalloc(&c->d_binom, c->h_binom.size() * 8));
+    c->dev_bytes += (i64)c->h_binom.size() * 8 + 96;
+    CU(cudaMemcpyAsync(c->d_binom, c->h_binom.data(), c->h_binom.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    const size_t eb = (size_t)(E ? E : 1);
+    CU(cudaMalloc(&c->d_dist, eb * 4));
+    CU(cudaMalloc(&c->d_edges, eb * 8));
+    CU(cudaMalloc(&c->d_K, eb * 4));
+    CU(cudaMalloc(&c->d_values, eb * 4));
+    c->dev_bytes += (i64)eb * 20;
+    c->n_distinct = 0;
+    if (E > 0) {
+        CU(cudaMemcpyAsync(c->d_dist, dist_lower, (size_t)E * 4, cudaMemcpyDefault, c->stream));
+        u64* tmp = nullptr;
+        CU(cudaMalloc(&tmp, (size_t)E * 8));
+        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+        CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+        CU(launch_prep_edges(c->d_dist, E, c->d_edges, (int*)(c->d_counters + 1), c->stream));
+        SortPlan plan = sort_make_plan(32, 64);
+        RC(ensure(c, c->sort_scratch, sort_scratch_bytes(E, plan)));
+        u64* res = nullptr;
+        cudaError_t e = sort_u64(c->d_edges, tmp, E, plan, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches);
+        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(e, "edge sort"); }
+        if (res != c->d_edges) { u64* t = c->d_edges; c->d_edges = res; tmp = t; }
+        DevBuf status;
+        int r = ensure(c, status, (size_t)rank_edges_tiles(E) * 8);
+        if (r != RIPS_OK) { cudaFree(tmp); return r; }
+        cudaMemsetAsync(status.p, 0, (size_t)rank_edges_tiles(E) * 8, c->stream);
+        e = launch_rank_edges(c->d_edges, E, c->d_K, c->d_values, (u64*)status.p, c->d_tickets, c->d_counters, c->stream);
+        c->launches += 2;
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        cudaFree(tmp);
+        release(c, status);
+        if (e != cudaSuccess) return cuda_fail(e, "edge ranking");
+        if ((int)c->h_counters[1] != 0) {
+            g_last_error = "rips_init: the distance matrix holds a NaN, negative or infinite entry";
+            return RIPS_EINVAL;
+        }
+        c->n_distinct = (u32)c->h_counters[0];
+        c->h_values.resize(c->n_distinct);
+        CU(cudaMemcpy(c->h_values.data(), c->d_values, (size_t)c->n_distinct * 4, cudaMemcpyDeviceToHost));
+    }
+    // keys are ranks in descending value order: thr_key = number of distinct values above the threshold
+    u32 lo = 0, hi = c->n_distinct;
+    while (lo < hi) {
+        u32 mid = (lo + hi) / 2;
+        if (c->h_values[mid] > c->threshold) lo = mid + 1;
+        else hi = mid;
+    }
+    c->thr_key = lo;
+    c->key_bits = bits_for(c->n_distinct ? c->n_distinct - 1 : 0);
+    (void)n;
+    return RIPS_OK;
+}
+
+} // namespace
+
+// =============================================================================================== C ABI
+extern "C" {
+
+const char* rips_strerror(int code)
+{
+    switch (code) {
+    case RIPS_OK: return "ok";
+    case RIPS_EINVAL: return "invalid argument";
+    case RIPS_EOVERFLOW: return "sizes overflow the 64-bit packed records";
+    case RIPS_ENOMEM: return "out of memory";
+    case RIPS_ECUDA: return "CUDA error";
+    default: return "unknown error";
+    }
+}
+
+const char* rips_last_error(void) { return g_last_error.c_str(); }
+
+int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes)
+{
+    if (!bytes || n < 1 || dim_max < 0 || dim_max > 4 || n >= 65536) return RIPS_EINVAL;
+    std::vector<u64> b;
+    build_binom(n, dim_max + 3, b);
+    auto C = [&](int k) { return b[(size_t)k * (n + 1) + n]; };
+    if (C(dim_max + 2) >> 62) return RIPS_EOVERFLOW;
+    long double total = 0;
+    const long double E = (long double)n * (n - 1) / 2;
+    total += E * 36 + (long double)b.size() * 8;
+    for (int d = 1; d <= dim_max; ++d) {
+        long double cand = (long double)C(d + 1);
+        // two column buffers, pair buffers (2) + non-apparent, bitmap, look-back words, sort scratch
+        total += cand * 8 * 5 + cand / 8 + cand / 4096 * 8 * 3 + cand / 8192 * 512 * 8 + (1 << 16);
+    }
+    if (total > 9.0e18L) return RIPS_EOVERFLOW;
+    *bytes = (int64_t)total;
+    return RIPS_OK;
+}
+
+int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* stream)
+{
+    g_last_error.clear();
+    if (!out) return RIPS_EINVAL;
+    *out = nullptr;
+    if (n < 1 || dim_max < 0 || dim_max > 4 || std::isnan(threshold)) return RIPS_EINVAL;
+    if (n >= 65536) return RIPS_EOVERFLOW;
+    if (n > 1 && !dist_lower) return RIPS_EINVAL;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        g_last_error = "no usable CUDA device: this library has no CPU fallback";
+        return RIPS_ECUDA;
+    }
+    rips_ctx* c = new (std::nothrow) rips_ctx();
+    if (!c) return RIPS_ENOMEM;
+    c->n = n;
+    c->E = n * (n - 1) / 2;
+    c->dim_max = dim_max;
+    c->threshold = threshold;
+    c->stream = (cudaStream_t)stream;
+    c->kmax = dim_max + 3;
+    build_binom(n, c->kmax, c->h_binom);
+    if (hbinom(c, n, dim_max + 2) >> 62) { delete c; return RIPS_EOVERFLOW; }
+    c->dims.resize((size_t)dim_max + 2);
+    int r = init_device_tables(c, dist_lower);
+    if (r == RIPS_OK) {
+        // the widest record of the requested dimensions must fit 64 bits
+        int cb = bits_for(hbinom(c, n, dim_max + 1) ? hbinom(c, n, dim_max + 1) - 1 : 0);
+        int tb = bits_for(hbinom(c, n, dim_max + 2) ? hbinom(c, n, dim_max + 2) - 1 : 0);
+        if (c->key_bits + cb > 64 || c->key_bits + tb > 64) r = RIPS_EOVERFLOW;
+    }
+    if (r != RIPS_OK) { rips_free(c); return r; }
+    *out = c;
+    return RIPS_OK;
+}
+
+void rips_free(rips_ctx* c)
+{
+    if (!c) return;
+    for (DimState& s : c->dims) free_dim(c, s);
+    release(c, c->sort_scratch);
+    release(c, c->d0_pairs);
+    release(c, c->d0_death);
+    release(c, c->d0_uf);
+    cudaFree(c->d_dist);
+    cudaFree(c->d_edges);
+    cudaFree(c->d_K);
+    cudaFree(c->d_values);
+    cudaFree(c->d_binom);
+    cudaFree(c->d_counters);
+    cudaFree(c->d_tickets);
+    if (c->h_counters) cudaFreeHost(c->h_counters);
+    cudaGetLastError();
+    delete c;
+}
+
+int rips_dim0(rips_ctx* c) { return c ? run_dim0(c) : RIPS_EINVAL; }
+int rips_stage1(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_stage1(c, d); }
+int rips_stage2(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_stage2(c, d); }
+int rips_reduce(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_reduce(c, d); }
+
+int rips_compute(rips_ctx* c)
+{
+    if (!c) return RIPS_EINVAL;
+    RC(run_dim0(c));
+    for (int d = 1; d <= c->dim_max; ++d) {
+        RC(run_stage1(c, d));
+        RC(run_stage2(c, d));
+        RC(run_reduce(c, d));
+    }
+    return RIPS_OK;
+}
+
+int rips_barcodes(rips_ctx* c, int d, const float** birth_death_host, int64_t* count)
+{
+    if (!c || !birth_death_host || !count || d < 0 || d > c->dim_max + 1) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_red) return RIPS_EINVAL;
+    *birth_death_host = s.bars.data();
+    *count = (int64_t)s.bars.size() / 2;
+    return RIPS_OK;
+}
+
+int rips_filtration(rips_ctx* c, int d, const float** diam_dev, const uint64_t** cidx_dev, int64_t* len)
+{
+    RC(check_dim(c, d, 1));
+    if (!diam_dev || !cidx_dev || !len) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s1) return RIPS_EINVAL;
+    if (!s.has_vf) {
+        RC(ensure(c, s.v_fdiam, (size_t)s.len * 4));
+        RC(ensure(c, s.v_fcidx, (size_t)s.len * 8));
+        CU(launch_unpack_columns(s.cols, s.len, s.cbits, c->d_values, (float*)s.v_fdiam.p, (u64*)s.v_fcidx.p, c->stream));
+        c->launches += s.len > 0;
+        CU(cudaStreamSynchronize(c->stream));
+        s.has_vf = true;
+    }
+    *diam_dev = (const float*)s.v_fdiam.p;
+    *cidx_dev = (const u64*)s.v_fcidx.p;
+    *len = s.len;
+    return RIPS_OK;
+}
+
+int rips_apparent_pairs(rips_ctx* c, int d, const uint64_t** t_dev, const uint64_t** s_dev, int64_t* n_app)
+{
+    RC(check_dim(c, d, 1));
+    if (!t_dev || !s_dev || !n_app) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s2) return RIPS_EINVAL;
+    if (!s.has_va) {
+        RC(ensure(c, s.v_at, (size_t)s.n_app * 8));
+        RC(ensure(c, s.v_as, (size_t)s.n_app * 8));
+        CU(launch_unpack_pairs(s.M, s.app, s.n_app, c->bt(), (int)c->n, (u64*)s.v_at.p, (u64*)s.v_as.p, c->stream));
+        c->launches += s.n_app > 0;
+        CU(cudaStreamSynchronize(c->stream));
+        s.has_va = true;
+    }
+    *t_dev = (const u64*)s.v_at.p;
+    *s_dev = (const u64*)s.v_as.p;
+    *n_app = s.n_app;
+    return RIPS_OK;
+}
+
+int rips_nonapparent(rips_ctx* c, int d, const float** diam_dev, const uint64_t** cidx_dev, int64_t* n_non)
+{
+    RC(check_dim(c, d, 1));
+    if (!diam_dev || !cidx_dev || !n_non) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s2) return RIPS_EINVAL;
+    if (!s.has_vn) {
+        RC(ensure(c, s.v_ndiam, (size_t)s.n_non * 4));
+        RC(ensure(c, s.v_ncidx, (size_t)s.n_non * 8));
+        CU(launch_unpack_columns((const u64*)s.non.p, s.n_non, s.cbits, c->d_values, (float*)s.v_ndiam.p,
+                                 (u64*)s.v_ncidx.p, c->stream));
+        c->launches += s.n_non > 0;
+        CU(cudaStreamSynchronize(c->stream));
+        s.has_vn = true;
+    }
+    *diam_dev = (const float*)s.v_ndiam.p;
+    *cidx_dev = (const u64*)s.v_ncidx.p;
+    *n_non = s.n_non;
+    return RIPS_OK;
+}
+
+int rips_pivots(rips_ctx* c, int d, const uint64_t** t_dev, const uint64_t** s_dev, int64_t* n_piv)
+{
+    RC(check_dim(c, d, 0));
+    if (!t_dev || !s_dev || !n_piv) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_red) return RIPS_EINVAL;
+    const i64 np = s.n_app + s.n_red;
+    if (!s.has_vp) {
+        RC(ensure(c, s.v_pt, (size_t)np * 8));
+        RC(ensure(c, s.v_ps, (size_t)np * 8));
+        CU(launch_merge_pivots(s.M, s.app, s.n_app, c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
+                               s.n_red, (u64*)s.v_pt.p, (u64*)s.v_ps.p, c->stream));
+        c->launches += np > 0;
+        CU(cudaStreamSynchronize(c->stream));
+        s.has_vp = true;
+    }
+    *t_dev = (const u64*)s.v_pt.p;
+    *s_dev = (const u64*)s.v_ps.p;
+    *n_piv = np;
+    return RIPS_OK;
+}
+
+int rips_pivot_lookup(rips_ctx* c, int d, const uint64_t* t_query_dev, int64_t m, int64_t* s_out_dev)
+{
+    RC(check_dim(c, d, 0));
+    if (m < 0 || (m > 0 && (!t_query_dev || !s_out_dev))) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s2) return RIPS_EINVAL;
+    CU(launch_pivot_lookup(s.M, s.app, s.n_app, c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
+                           s.have_red ? s.n_red : 0, t_query_dev, m, s_out_dev, c->stream));
+    c->launches += m > 0;
+    CU(cudaStreamSynchronize(c->stream));
+    return RIPS_OK;
+}
+
+int rips_stats(rips_ctx* c, int d, rips_stats_t* out)
+{
+    RC(check_dim(c, d, 0));
+    if (!out) return RIPS_EINVAL;
+    *out = c->dims[d].stats;
+    return RIPS_OK;
+}
+
+int rips_timings(rips_ctx* c, int d, rips_timings_t* out)
+{
+    RC(check_dim(c, d, 0));
+    if (!out) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    CU(cudaStreamSynchronize(c->stream));
+    rips_timings_t t = s.tim;
+    t.clear_bitmap_ms = ev_ms(s, EV_S1_BEGIN, EV_S1_BITMAP);
+    t.enumerate_ms = ev_ms(s, EV_S1_BITMAP, EV_S1_ENUM);
+    t.sort_hist_ms = ev_ms(s, EV_S1_SORTBEG, EV_S1_HIST);
+    t.sort_pass_ms = ev_ms(s, EV_S1_HIST, EV_S1_SORT);
+    t.stage1_ms = ev_ms(s, EV_S1_BEGIN, EV_S1_END);
+    t.apparent_ms = ev_ms(s, EV_S2_BEGIN, EV_S2_APP);
+    t.pair_hist_ms = ev_ms(s, EV_S2_SORTBEG, EV_S2_HIST);
+    t.pair_sort_ms = ev_ms(s, EV_S2_HIST, EV_S2_SORT);
+    t.stage2_ms = ev_ms(s, EV_S2_BEGIN, EV_S2_END);
+    t.dim0_ms = ev_ms(s, EV_D0_BEGIN, EV_D0_END);
+    *out = t;
+    return RIPS_OK;
+}
+
+int rips_device_bytes(rips_ctx* c, int64_t* bytes)
+{
+    if (!c || !bytes) return RIPS_EINVAL;
+    *bytes = c->dev_bytes;
+    return RIPS_OK;
+}
+
+int rips_kernel_launches(rips_ctx* c, int64_t* launches)
+{
+    if (!c || !launches) return RIPS_EINVAL;
+    *launches = c->launches;
+    return RIPS_OK;
+}
+
+int rips_sort_u64(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, int hi_bit, void* stream)
+{
+    g_last_error.clear();
+    if (n < 0 || lo_bit < 0 || hi_bit > 64 || lo_bit >= hi_bit || (n > 0 && (!keys_dev || !tmp_dev))) return RIPS_EINVAL;
+    if (n <= 1) return RIPS_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    SortPlan plan = sort_make_plan(lo_bit, hi_bit);
+    void* scratch = nullptr;
+    cudaError_t e = cudaMalloc(&scratch, sort_scratch_bytes(n, plan));
+    if (e != cudaSuccess) { cudaGetLastError(); return RIPS_ENOMEM; }
+    u64* res = nullptr;
+    e = sort_u64(keys_dev, tmp_dev, n, plan, scratch, st, &res, nullptr, nullptr);
+    if (e == cudaSuccess && res != keys_dev)
+        e = cudaMemcpyAsync(keys_dev, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "rips_sort_u64");
+    return RIPS_OK;
+}
+
+} // extern "C"
