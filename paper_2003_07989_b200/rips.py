@@ -105,7 +105,7 @@ class _DevView:
     """__cuda_array_interface__ wrapper of a raw device pointer (zero-copy view for torch.as_tensor)."""
 
     def __init__(self, ptr, count, typestr):
-        self.__cuda_array_interface__ = {"shape": (int(count),), "typestr": typestr, "data": (int(ptr), True),
+        self.__cuda_array_interface__ = {"shape": (int(count),), "typestr": typestr, "data": (int(ptr), False),
                                          "version": 2}
 
 

@@ -1,0 +1,144 @@
+"""GPU parity: the CUDA path, called through the C ABI (paper_2003_07989_b200.rips), against the CPU
+oracle (oracle/), element by element and bit-exact, on the same seeded inputs.  Every output is
+integer / index data or a selected fp32 input value, so the tolerance is zero."""
+from math import comb, inf
+
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2003_07989_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def R():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2003_07989_b200 import rips
+    rips.lib()
+    return rips
+
+
+def _np(t):
+    return t.cpu().numpy()
+
+
+def check_against_oracle(R, low, n, dim_max, thr=inf, what=""):
+    o = oracle.barcodes(low, n, dim_max, thr)
+    with R.Rips(low, n, dim_max, thr) as g:
+        g.compute()
+        # dimension 0
+        pt, ps = g.pivots(0)
+        assert np.array_equal(_np(pt).astype(np.uint64), o[0]["pivot_t"]), what
+        assert np.array_equal(_np(ps).astype(np.uint64), o[0]["pivot_s"]), what
+        assert np.array_equal(g.barcodes(0), o[0]["bars"].reshape(-1, 2)), what
+        for d in range(1, dim_max + 1):
+            tag = f"{what} d={d}"
+            fd, fc = g.filtration(d)
+            assert np.array_equal(_np(fc).astype(np.uint64), o[d]["filt_cidx"]), tag
+            assert np.array_equal(_np(fd).view(np.uint32), o[d]["filt_diam"].view(np.uint32)), tag
+            at, as_ = g.apparent_pairs(d)
+            assert np.array_equal(_np(at).astype(np.uint64), o[d]["app_t"]), tag
+            assert np.array_equal(_np(as_).astype(np.uint64), o[d]["app_s"]), tag
+            nd, nc = g.nonapparent(d)
+            assert np.array_equal(_np(nc).astype(np.uint64), o[d]["non_cidx"]), tag
+            assert np.array_equal(_np(nd).view(np.uint32), o[d]["non_diam"].view(np.uint32)), tag
+            pt, ps = g.pivots(d)
+            assert np.array_equal(_np(pt).astype(np.uint64), o[d]["pivot_t"]), tag
+            assert np.array_equal(_np(ps).astype(np.uint64), o[d]["pivot_s"]), tag
+            assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32)), tag
+            st = g.stats(d)
+            c = o[d]["counts"]
+            assert st["n_candidates"] == comb(n, d + 1)
+            assert (st["n_columns"], st["n_removed_by_diameter"], st["n_cleared"]) == \
+                   (c["kept"], c["removed_by_diameter"], c["cleared"]), tag
+            assert st["n_apparent"] == o[d]["app_t"].size and st["n_nonapparent"] == o[d]["non_cidx"].size
+            assert st["n_essential"] == o[d]["essential"].size
+            # a10: lookup of every pivot row, and of rows that are not pivots
+            if o[d]["pivot_t"].size:
+                q = o[d]["pivot_t"][:: max(1, o[d]["pivot_t"].size // 500)]
+                got = _np(g.pivot_lookup(d, q.astype(np.int64)))
+                want = o[d]["pivot_s"][:: max(1, o[d]["pivot_t"].size // 500)].astype(np.int64)
+                assert np.array_equal(got, want), tag
+            allrows = np.arange(min(comb(n, d + 2), 2000), dtype=np.int64)
+            isp = np.isin(allrows.astype(np.uint64), o[d]["pivot_t"])
+            got = _np(g.pivot_lookup(d, allrows))
+            assert np.array_equal(got >= 0, isp), tag
+
+
+@pytest.mark.parametrize("k,n", [(1, 12), (2, 14), (3, 16), (4, 40), (5, 18), (1, 50), (2, 40), (3, 60), (5, 48)])
+def test_shadow_configs(R, k, n):
+    w = inputs.config(k, n)
+    thr = w.threshold if k != 5 else inputs.enclosing_radius(w.dist, n)
+    if k == 4:
+        thr = float(np.float32(np.quantile(w.dist, 0.25)))
+    check_against_oracle(R, w.dist, n, w.dim_max, thr, w.name)
+
+
+@pytest.mark.parametrize("name", ["constant", "cyclic", "cross", "descending", "smallint", "zeros"])
+def test_degenerate_value_patterns(R, name):
+    n = 13
+    low = {"constant": inputs.constant_lower(n), "cyclic": inputs.cyclic_lower(n),
+           "cross": inputs.cross_polytope_lower(6), "descending": inputs.descending_lower(n),
+           "smallint": inputs.small_integer_lower(n, 7),
+           "zeros": inputs.euclidean_lower(np.repeat(inputs.cube_points(5, 2, 1), 3, axis=0)[:n])}[name]
+    nn = 12 if name == "cross" else n
+    check_against_oracle(R, low, nn, 3 if name != "zeros" else 2, inf, name)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4])
+def test_tiny_n(R, n):
+    low = inputs.random_matrix_lower(n, 3)
+    check_against_oracle(R, low, n, 2, inf, f"n={n}")
+    check_against_oracle(R, low + 1.0, n, 2, 0.5, f"n={n} below every distance")
+
+
+def test_threshold_sweep(R):
+    w = inputs.config(1, 30)
+    for q in (0.0, 0.1, 0.5, 0.9, 1.0):
+        thr = float(np.float32(np.quantile(w.dist, q)))
+        check_against_oracle(R, w.dist, 30, 2, thr, f"q={q}")
+
+
+def test_config1_full(R):
+    w = inputs.config(1)
+    check_against_oracle(R, w.dist, w.n, w.dim_max, w.threshold, w.name)
+
+
+def test_sort_primitive(R):
+    import torch
+    rng = np.random.default_rng(11)
+    for n, lo, hi in [(1, 0, 8), (2, 3, 20), (1000, 0, 64), (8192, 5, 22), (8193, 0, 9), (100003, 13, 30),
+                      (1 << 20, 40, 57), (300007, 0, 1)]:
+        a = rng.integers(0, 1 << 63, n, dtype=np.int64) * 2 + rng.integers(0, 2, n, dtype=np.int64)
+        if n == 100003:
+            a[:] = a[0]                       # all keys equal: must come back untouched (stability)
+            a += np.arange(n) << 32
+        t = torch.from_numpy(a).cuda()
+        R.rips_sort_u64(t, lo, hi)
+        u = a.view(np.uint64)
+        key = (u >> np.uint64(lo)) & np.uint64((1 << (hi - lo)) - 1)
+        want = u[np.argsort(key, kind="stable")]
+        assert np.array_equal(t.cpu().numpy().view(np.uint64), want), (n, lo, hi)
+
+
+def test_invalid_inputs(R):
+    bad = np.array([1.0, np.nan, 2.0], dtype=np.float32)
+    for arr in (bad, np.array([1.0, -2.0, 2.0], dtype=np.float32), np.array([1.0, np.inf, 2.0], dtype=np.float32)):
+        with pytest.raises(R.RipsError) as e:
+            R.Rips(arr, 3, 1)
+        assert e.value.code == R.RIPS_EINVAL
+    with pytest.raises(R.RipsError):
+        R.Rips(np.ones(3, dtype=np.float32), 3, 7)
+    with pytest.raises(R.RipsError):
+        R.Rips(np.ones(3, dtype=np.float32), 3, 1, float("nan"))
+    g = R.Rips(np.ones(3, dtype=np.float32), 3, 1)
+    with pytest.raises(R.RipsError):
+        g.stage2(1)                           # stage 1 has not run
+    neg0 = np.array([-0.0, 1.0, 1.0], dtype=np.float32)
+    check_against_oracle(R, np.abs(neg0), 3, 1)
+    with R.Rips(neg0, 3, 1) as h:
+        h.compute()
+        assert np.array_equal(h.barcodes(0), oracle.barcodes(np.abs(neg0), 3, 1)[0]["bars"].reshape(-1, 2))
