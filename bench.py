@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Vietoris-Rips hot path (filtration construction with clearing
++ apparent pairs) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A "step" is one pass of the whole hot path (every row a3-a10 of DESIGN.md section 1) over one
+workload: for d = 1..dim_max: rips_stage1(d) (enumerate + diameter + threshold + clearing +
+compaction + onesweep sort), rips_stage2(d) (apparent-pair kernel + partition + pair sort), called
+through the C ABI on a context whose distance matrix, key matrix, binomial table and clearing sets
+are resident in HBM (one untimed rips_compute produced them).  `value` = candidate simplices
+(sum over d of C(n, d+1)) per second, whole job.  `e2e` = the same count divided by the time of
+rips_init (HOST distance matrix) + rips_compute (dim 0, both stages, reduction) + rips_barcodes
+(HOST bars), copies inside the timed region.  The serial remainder (dim 0, reduction of the
+non-apparent columns) is reported separately under "barcode".
+
+Multi-GPU: replicas only -- every rank runs the same workload on its own
+GPU, no data-path collective; timing is the max over ranks.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+from math import comb
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "simplices/sec (filtration+clearing+apparent pairs)"
+UNIT = "simplices/s"
+RECORD_BYTES = 8  # packed column / pair record
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k-1]; 2 is the one the metric is quoted on")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--warmup-seconds", type=float, default=0.6,
+                    help="keep warming up until this much time has passed (gives the clock sampler load to see)")
+    return ap.parse_args()
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload_dict(w, n_cand):
+    thr = None if w.threshold == float("inf") else w.threshold
+    return {"workload": w.name, "n": w.n, "dim_max": w.dim_max, "threshold": thr, "note": w.note,
+            "candidates_per_step": n_cand,
+            "l2": "no flush: the record arrays of the top dimension exceed the 126 MB L2"}
+
+
+# ------------------------------------------------------------------------------------ CPU oracle leg
+def oracle_sample(w, budget_s):
+    """The oracle as it stands (stage 1 + stage 2 of every dimension) on a bounded sample: the lower
+    dimensions completely, then slices of the top dimension's index range until the budget is used.
+    Returns (simplices, seconds, cores, description)."""
+    from oracle import oracle
+    t_all = time.perf_counter()
+    z = oracle.dim0(w.dist, w.n, w.threshold)
+    cleared = z["t"]
+    done, spent, parts = 0, 0.0, []
+    for d in range(1, w.dim_max + 1):
+        total = comb(w.n, d + 1)
+        if d < w.dim_max:
+            t0 = time.perf_counter()
+            fd, fc, _ = oracle.stage1(w.dist, w.n, d, w.threshold, cleared)
+            s2 = oracle.stage2(w.dist, w.n, d, fd, fc)
+            spent += time.perf_counter() - t0
+            done += total
+            parts.append(f"d={d} all {total}")
+            # clearing set of the next dimension (untimed: the reduction is not the hot path)
+            red = oracle.reduce_columns(w.dist, w.n, d, w.threshold, s2["non_cidx"], s2["app_t"], s2["app_s"])
+            cleared = np.sort(np.concatenate([s2["app_t"], red["t"]]))
+        else:
+            lo, chunk = 0, 2_000_000
+            while lo < total and (spent < budget_s or lo == 0):
+                hi = min(total, lo + chunk)
+                t0 = time.perf_counter()
+                fd, fc, _ = oracle.stage1(w.dist, w.n, d, w.threshold, cleared, lo, hi)
+                oracle.stage2(w.dist, w.n, d, fd, fc)
+                spent += time.perf_counter() - t0
+                done += hi - lo
+                lo = hi
+            parts.append(f"d={d} candidates [0,{lo}) of {total}")
+    desc = "oracle stage 1 + stage 2 (sort included): " + "; ".join(parts)
+    return done, spent, oracle.num_threads(), desc, time.perf_counter() - t_all
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2003_07989_b200 import inputs
+    w = inputs.config(args.config)
+    n_cand = sum(comb(w.n, d + 1) for d in range(1, w.dim_max + 1))
+    per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(w, per_step / 4)
+    tot_s, tot_t, cores, desc = 0, 0.0, 0, ""
+    for _ in range(args.steps):
+        s, t, cores, desc, _ = oracle_sample(w, per_step)
+        tot_s += s
+        tot_t += t
+    value = tot_s / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": workload_dict(w, n_cand),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------ clocks sampler
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms DURING the timed region (B200_PROFILING.md's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        with open(self.path) as f:
+            for ln in f:
+                p = [x.strip() for x in ln.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1])); smax.append(float(p[2])); power.append(float(p[3]))
+                except ValueError:
+                    continue
+                for name, v in zip(names, p[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        os.unlink(self.path)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "power_w_max": max(power),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------ B200 arm
+KERNELS = {  # rips_timings field -> (kernel, launches per stage call, algorithmic bytes per launch)
+    "enumerate_ms": "stage1_kernel (a3-a5 enumerate+filter+compact)",
+    "sort_pass_ms": "onesweep_pass_kernel (a6 filtration sort)",
+    "apparent_ms": "stage2_kernel (a7-a8 apparent pairs+partition)",
+    "pair_sort_ms": "onesweep_pass_kernel (a9 pair sort)",
+}
+
+
+def algorithmic_bytes(field, st):
+    """HBM bytes ONE launch of the kernel must move, from rips_stats of that dimension."""
+    if field == "enumerate_ms":   # clearing bitmap read + survivors written
+        return st["n_candidates"] / 8 + RECORD_BYTES * st["n_columns"], 1
+    if field == "sort_pass_ms":   # each pass reads and writes every record once
+        return 2 * RECORD_BYTES * st["n_columns"], max(1, st["sort_passes"])
+    if field == "apparent_ms":    # columns read, pairs + non-apparent columns written
+        return RECORD_BYTES * (st["n_columns"] + st["n_apparent"] + st["n_nonapparent"]), 1
+    if field == "pair_sort_ms":
+        return 2 * RECORD_BYTES * st["n_apparent"], max(1, st["pair_sort_passes"])
+    raise KeyError(field)
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product has no CPU fallback"
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2003_07989_b200 import inputs, rips
+    rips.lib()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = inputs.config(args.config)
+    D = w.dim_max
+    n_cand = sum(comb(w.n, d + 1) for d in range(1, D + 1))
+    host = torch.from_numpy(w.dist).pin_memory()
+    dev = host.cuda()
+
+    # ---- resident context; one full computation provides the clearing sets (and the barcode time)
+    g = rips.Rips(dev, w.n, D, w.threshold)
+    t0 = time.perf_counter()
+    g.compute()
+    torch.cuda.synchronize()
+    first_compute_ms = 1e3 * (time.perf_counter() - t0)
+    stats = {d: g.stats(d) for d in range(0, D + 1)}
+
+    def hot_step():
+        for d in range(1, D + 1):
+            g.stage1(d)
+            g.stage2(d)
+
+    # ---- clocks are sampled from the warm-up on (nvidia-smi needs ~0.2 s to start) through the timed region
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    t_w = time.perf_counter()
+    n_w = 0
+    while n_w < max(args.warmup, 3) or (time.perf_counter() - t_w < args.warmup_seconds and n_w < 200):
+        hot_step()
+        n_w += 1
+    per_kernel = {k: 0.0 for k in KERNELS}
+    per_kernel_dim = {k: {d: 0.0 for d in range(1, D + 1)} for k in KERNELS}
+    stage_ms = 0.0
+    launches0 = g.kernel_launches()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        hot_step()
+        for d in range(1, D + 1):   # events recorded by the library on the same stream; already complete
+            t = g.timings(d)
+            for k in KERNELS:
+                per_kernel[k] += t[k]
+                per_kernel_dim[k][d] += t[k]
+            stage_ms += t["stage1_ms"] + t["stage2_ms"]
+    ev1.record()
+    barrier()
+    elapsed_ms = ev0.elapsed_time(ev1)
+    launches = g.kernel_launches() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        tt = torch.tensor([elapsed_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(tt.item())
+    ms_per_step = elapsed_ms / args.steps
+    value = world * n_cand / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (largest share of the timed region)
+    peak, peak_src = load_peaks()
+    kernels = []
+    for k, name in KERNELS.items():
+        d_top = max(per_kernel_dim[k], key=lambda d: per_kernel_dim[k][d])
+        b, nl = algorithmic_bytes(k, g.stats(d_top))
+        ms_launch = per_kernel_dim[k][d_top] / args.steps / nl
+        kernels.append({"kernel": name, "dim": d_top, "ms_per_step_all_dims": per_kernel[k] / args.steps,
+                        "ms_per_launch": ms_launch, "launches_per_step": nl, "bytes_per_launch": b,
+                        "gbs": (b / (ms_launch * 1e-3) / 1e9) if ms_launch > 0 else 0.0,
+                        "frac_of_peak": (b / (ms_launch * 1e-3) / 1e9 / peak) if ms_launch > 0 else 0.0,
+                        "share_of_step": per_kernel[k] / args.steps / ms_per_step})
+    top = max(kernels, key=lambda r: r["ms_per_step_all_dims"])
+    roofline = {"bound": "hbm", "kernel": top["kernel"], "dim": top["dim"], "achieved": top["gbs"], "peak": peak,
+                "unit": "GB/s", "frac": top["frac_of_peak"], "traffic": None, "peak_source": peak_src,
+                "bytes_per_launch": top["bytes_per_launch"], "ms_per_launch": top["ms_per_launch"],
+                "nominal_peak_gbs": 8000.0, "frac_of_nominal": top["gbs"] / 8000.0}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            tj = json.load(f)
+        key = f"cfg{args.config}:{top['kernel'].split(' ')[0]}:{'a9' if 'a9' in top['kernel'] else 'a6' if 'a6' in top['kernel'] else ''}"
+        roofline["traffic"] = tj.get(key)
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    e2e_ms, d2h_bytes, parts = [], 0, None
+    for i in range(args.e2e_steps + 1 if args.e2e_steps > 0 else 0):
+        barrier()
+        t0 = time.perf_counter()
+        h = rips.Rips(host.numpy(), w.n, D, w.threshold)
+        h.compute()
+        bars = [h.barcodes(d) for d in range(0, D + 1)]
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        if i > 0:   # the first one warms the allocator
+            e2e_ms.append(1e3 * (t1 - t0))
+        d2h_bytes = sum(b.nbytes for b in bars)
+        tim = {d: h.timings(d) for d in range(0, D + 1)}
+        parts = {"dim0_ms": tim[0]["dim0_ms"],
+                 "hot_path_ms": sum(tim[d]["stage1_ms"] + tim[d]["stage2_ms"] for d in range(1, D + 1)),
+                 "reduce_host_ms": sum(tim[d]["reduce_host_ms"] for d in range(1, D + 1)),
+                 "reduce_xfer_ms": sum(tim[d]["reduce_xfer_ms"] for d in range(1, D + 1)),
+                 "bars": {str(d): int(b.shape[0]) for d, b in enumerate(bars)}}
+        h.free()
+    e2e_t = statistics.median(e2e_ms) if e2e_ms else float("nan")
+    if world > 1:
+        tt = torch.tensor([e2e_t], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_t = float(tt.item())
+    e2e = {"value": world * n_cand / (e2e_t * 1e-3), "unit": UNIT, "ms": e2e_t,
+           "h2d_bytes_per_step": int(host.numel() * 4), "d2h_bytes_per_step": int(d2h_bytes),
+           "what": "rips_init(host matrix) + rips_compute + rips_barcodes(host) + rips_free"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        s, t, cores, desc, _ = oracle_sample(w, args.cpu_seconds)
+        cpu = {"value": s / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": n_w, "ms_per_step": ms_per_step, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+                "config": workload_dict(w, n_cand), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu,
+                "kernels": kernels,
+                "barcode": {"end_to_end_ms": e2e_t, "first_compute_ms": first_compute_ms, **(parts or {})},
+                "stats": {str(d): {k: stats[d][k] for k in ("n_candidates", "n_columns", "n_cleared",
+                                                            "n_removed_by_diameter", "n_apparent", "n_nonapparent",
+                                                            "sort_passes", "pair_sort_passes", "key_bits",
+                                                            "index_bits")} for d in range(1, D + 1)},
+                "device_bytes": g.device_bytes(), "parallelism": "replicas" if world > 1 else "single"}
+        print(json.dumps(line))
+    g.free()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

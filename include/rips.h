@@ -105,7 +105,9 @@ int rips_compute(rips_ctx* ctx);
 /* The two hot-path stages, separately callable for d in [1, dim_max+1] (benches, and the scale row
  * of DESIGN.md: stage 1 at d = dim_max+1 enumerates the C(n, dim_max+2) simplices the configs
  * name).  rips_stage1(d) needs the pivots of dimension d-1 (rips_compute, or rips_dim0 for d = 1);
- * rips_stage2(d) needs rips_stage1(d).  Both may be called repeatedly. */
+ * rips_stage2(d) needs rips_stage1(d).  Both may be called repeatedly: the pivots an earlier
+ * rips_reduce(d) found depend only on the input and stay valid, so after one rips_compute the loop
+ * "for d: rips_stage1(d); rips_stage2(d)" re-runs the whole hot path (bench.py's step). */
 int rips_dim0(rips_ctx* ctx);
 int rips_stage1(rips_ctx* ctx, int d);
 int rips_stage2(rips_ctx* ctx, int d);

@@ -257,15 +257,26 @@ int run_stage1(rips_ctx* c, int d)
     if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     DimState& prev = c->dims[d - 1];
-    if (!prev.have_red) { g_last_error = "rips_stage1: pivots of the previous dimension are missing"; return RIPS_EINVAL; }
+    if (!prev.have_red || !prev.have_s2) {
+        g_last_error = "rips_stage1: pivots of the previous dimension are missing";
+        return RIPS_EINVAL;
+    }
     const i64 n = c->n;
     s.M = d + 1;
     s.total = hbinom(c, n, d + 1);
     s.cbits = bits_for(s.total ? s.total - 1 : 0);
     if (c->key_bits + s.cbits > 64) return RIPS_EOVERFLOW;
-    s.have_s1 = s.have_s2 = s.have_red = false;
+    // The pivots found by an earlier rips_reduce(d) depend only on the input, so they stay valid
+    // (have_red) while stage 1 / stage 2 are re-run; accessors additionally require have_s2.
+    s.have_s1 = s.have_s2 = false;
     invalidate_views(s, true, true, true, true);
     rips_stats_t keep_stats = rips_stats_t{};
+    if (s.have_red) {
+        keep_stats.n_reduced_pivots = s.stats.n_reduced_pivots;
+        keep_stats.n_essential = s.stats.n_essential;
+        keep_stats.n_additions = s.stats.n_additions;
+        keep_stats.n_bars = s.stats.n_bars;
+    }
     s.stats = keep_stats;
     s.stats.n_candidates = (i64)s.total;
     s.stats.key_bits = c->key_bits;
@@ -367,7 +378,7 @@ int run_stage2(rips_ctx* c, int d)
     if (rows == ~0ull) return RIPS_EOVERFLOW;
     s.tbits = bits_for(rows ? rows - 1 : 0);
     if (s.tbits + RIPS_PAIR_POS_BITS > 64 || s.tbits + c->key_bits > 64) return RIPS_EOVERFLOW;
-    s.have_s2 = s.have_red = false;
+    s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
     s.n_app = s.n_non = 0;
     s.app = nullptr;
@@ -700,7 +711,7 @@ int rips_barcodes(rips_ctx* c, int d, const float** birth_death_host, int64_t* c
 {
     if (!c || !birth_death_host || !count || d < 0 || d > c->dim_max + 1) return RIPS_EINVAL;
     DimState& s = c->dims[d];
-    if (!s.have_red) return RIPS_EINVAL;
+    if (!s.have_red || !s.have_s2) return RIPS_EINVAL;
     *birth_death_host = s.bars.data();
     *count = (int64_t)s.bars.size() / 2;
     return RIPS_OK;
@@ -772,7 +783,7 @@ int rips_pivots(rips_ctx* c, int d, const uint64_t** t_dev, const uint64_t** s_d
     RC(check_dim(c, d, 0));
     if (!t_dev || !s_dev || !n_piv) return RIPS_EINVAL;
     DimState& s = c->dims[d];
-    if (!s.have_red) return RIPS_EINVAL;
+    if (!s.have_red || !s.have_s2) return RIPS_EINVAL;
     const i64 np = s.n_app + s.n_red;
     if (!s.has_vp) {
         RC(ensure(c, s.v_pt, (size_t)np * 8));
