@@ -76,18 +76,18 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, i64 tile, u64 agg
 }
 
 // ---------------------------------------------------------------------------------------------
-// Compressed distance matrix of diameter KEYS.  key(e) = dense rank of the edge value in
-// DESCENDING order (0 = the largest distance), so diam(simplex) = max value = MIN key, the
-// coboundary order (diameter descending) is key ascending, and "diam <= threshold" is
-// "key >= thr_key".  Element (a > b) at a(a-1)/2 + b.
+// Diameter KEYS.  key(e) = dense rank of the edge value in DESCENDING order (0 = the largest
+// distance), so diam(simplex) = max value = MIN key, the coboundary order (diameter descending) is
+// key ascending, and "diam <= threshold" is "key >= thr_key".
+//   K  : u32, strict lower triangle, element (a > b) at a(a-1)/2 + b          (set-up, host reduction)
+//   Kf : full symmetric n x n matrix of key+1 with a ZERO diagonal, u16 when every key+1 fits,
+//        else u32.  The shift makes 0 smaller than every real entry, so a test "all edges from v
+//        to the vertices of s have key >= key(s)" rejects v in s by itself, with no membership
+//        logic, and rows are contiguous in the scanned vertex whichever of the two is larger.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ u32 dkey(const u32* __restrict__ K, int a, int b)
 {
     int hi = max(a, b), lo = min(a, b);
-    return __ldg(K + ((u32)hi * (u32)(hi - 1) >> 1) + lo);
-}
-__device__ __forceinline__ u32 dkey_ordered(const u32* __restrict__ K, int hi, int lo)
-{
     return __ldg(K + ((u32)hi * (u32)(hi - 1) >> 1) + lo);
 }
 
@@ -118,6 +118,39 @@ __device__ __forceinline__ void decode_simplex(const BinomTable& bt, u64 idx, in
 #pragma unroll
     for (int k = M; k >= 1; --k) {
         int x = binom_upper_vertex(bt, idx, k, k - 1, hi);
+        v[k - 1] = x;
+        idx -= bt(x, k);
+        hi = x - 1;
+    }
+}
+
+// Same result as decode_simplex, but each binary search is replaced by the closed-form estimate
+// v ~ (k! idx)^(1/k) + (k-1)/2 (from C(v,k) ~ (v-(k-1)/2)^k / k!) followed by an exact fix-up against
+// the table, so the float arithmetic only decides how many fix-up steps run, never the result.
+template <int M>
+__device__ __forceinline__ void decode_simplex_fast(const BinomTable& bt, u64 idx, int n, int (&v)[M])
+{
+    int hi = n - 1;
+#pragma unroll
+    for (int k = M; k >= 1; --k) {
+        int x;
+        if (k == 1) {
+            x = (int)idx;
+        } else {
+            float fact = 1.f;
+#pragma unroll
+            for (int i = 2; i <= k; ++i) fact *= (float)i;
+            const float y = fact * (float)idx;
+            float r;
+            if (k == 2) r = sqrtf(y);
+            else if (k == 4) r = sqrtf(sqrtf(y));
+            else r = __powf(y, 1.0f / (float)k);
+            x = (int)(r + 0.5f * (float)(k - 1));
+            x = min(max(x, k - 1), hi);
+            const u64* row = bt.B + k * bt.stride;
+            while (x < hi && __ldg(row + x + 1) <= idx) ++x;
+            while (x > k - 1 && __ldg(row + x) > idx) --x;
+        }
         v[k - 1] = x;
         idx -= bt(x, k);
         hi = x - 1;

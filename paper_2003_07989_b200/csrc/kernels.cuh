@@ -1,8 +1,13 @@
 // kernels.cuh -- host-side launchers of the hot-path kernels (definitions in stage1.cu, stage2.cu,
 // dim0.cu, init.cu).  Packed records used throughout the device path:
 //
-//   column record   (key << cbits) | cidx      key = descending dense rank of the diameter
-//                                               (0 = largest distance), cbits = bits of C(n,d+1)-1
+//   column record   (key << lowbits) | verts   key = descending dense rank of the diameter (0 = largest
+//                                               distance); verts = the simplex's vertices, v[j] at bit
+//                                               j*vbits, vbits = bits of n-1, lowbits = (d+1)*vbits.
+//                                               The vertex word orders simplices exactly like cidx does
+//                                               (colex order = lexicographic on the decreasing vertex
+//                                               tuple, Remark 2), and spares stage 2 and
+//                                               the unpack kernels the inverse of Eq. 2.
 //   pair record     (cidx(t) << 3) | j         j = position of the added vertex v inside t
 //                                               (number of vertices of s below v); s = t minus that vertex
 //
@@ -22,6 +27,8 @@ cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, cudaStream
 cudaError_t launch_rank_edges(const u64* rec_sorted, i64 E, u32* K, float* values, u64* status, u32* ticket,
                               u64* n_distinct, cudaStream_t st);
 i64 rank_edges_tiles(i64 E);
+// Kf (see common.cuh) from K: n*n entries of u16 (kf_u16 != 0) or u32
+cudaError_t launch_build_full_keys(const u32* K, int n, void* Kf, int kf_u16, cudaStream_t st);
 
 // ------------------------------------------------------------------ dim0.cu
 struct Dim0Out {
@@ -41,21 +48,29 @@ struct ClearSet {
     const u64* layer2;     // sorted t of the reduced pivots
     i64 n2;
 };
+// digits of a radix sort whose histogram a producer kernel accumulates while it writes the records
+struct FusedHist {
+    u64* hist;        // [npasses][256] raw counts, zeroed by the caller; NULL = not fused
+    int npasses;      // <= 4
+    int shift[4], bits[4];
+};
 struct Stage1Params {
-    const u32* K;
+    const void* Kf;   // full key matrix (u16 or u32, see launch_stage1's kf_u16)
     BinomTable bt;
     int n;
     u64 total;        // C(n, d+1)
+    i64 tiles;
     u32 thr_key;      // keep iff key >= thr_key
-    int cbits;
+    int vbits, lowbits;
     ClearSet clear;
     u64* out;         // packed column records in increasing cidx; NULL = count only
     u64* status;      // one word per tile, zeroed
     u32* ticket;      // zeroed
     u64* counters;    // [0] kept [1] removed by diameter [2] cleared ; zeroed
+    FusedHist fh;     // histogram of the filtration sort's digits
 };
 i64 stage1_tiles(u64 total);
-cudaError_t launch_stage1(int M, const Stage1Params& p, cudaStream_t st);
+cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
 // bitmap |= bits of the given pivot rows
 cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, cudaStream_t st);
 
@@ -63,23 +78,26 @@ cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int sh
 struct Stage2Params {
     const u64* cols;  // sorted packed column records
     i64 len;
-    const u32* K;
+    const void* Kf;
     BinomTable bt;
     int n;
-    int cbits;
-    u64* app_out;     // packed pair records, in column order (sorted by t afterwards)
-    u64* non_out;     // packed column records of the non-apparent columns, in column order
-    u64* status_app;  // one word per tile each, zeroed
-    u64* status_non;
-    u32* ticket;      // zeroed
-    u64* counters;    // [0] apparent [1] non-apparent ; zeroed
+    int vbits, lowbits;
+    int kmax;         // rows of the binomial table (k = 0..kmax)
+    u64* app_out;     // one record per column (pair record or sentinel), sorted by t afterwards
+    u64* counters;    // [0] apparent ; zeroed
 };
 i64 stage2_tiles(i64 len);
-cudaError_t launch_stage2(int M, const Stage2Params& p, cudaStream_t st);
+// app_out gets one record per column: the pair record, or `sentinel` for a non-apparent column;
+// nonmask: ceil(len/32) words, bit set <=> column is not apparent.  counters[0] += apparent.
+cudaError_t launch_stage2(int M, int kf_u16, const Stage2Params& p, u64 sentinel, u32* nonmask, cudaStream_t st);
+// ordered gather of the non-apparent columns; *counter += their number; status: stage2_tiles(len) words, zeroed
+cudaError_t launch_compact_nonapparent(const u32* nonmask, i64 len, const u64* cols, u64* non_out, u64* status, u32* ticket,
+                                       u64* counter, cudaStream_t st);
 
 // ------------------------------------------------------------------ unpack / lookup (stage2.cu)
-cudaError_t launch_unpack_columns(const u64* cols, i64 len, int cbits, const float* values, float* diam, u64* cidx,
-                                  cudaStream_t st);
+// packed column records -> diam[], cidx[] (M = vertices of the simplex; cidx by Eq. 2)
+cudaError_t launch_unpack_columns(int M, const u64* cols, i64 len, int vbits, BinomTable bt, const float* values,
+                                  float* diam, u64* cidx, cudaStream_t st);
 // packed pair records -> t[], s[]   (M = vertices of s)
 cudaError_t launch_unpack_pairs(int M, const u64* pairs, i64 len, BinomTable bt, int n, u64* t, u64* s, cudaStream_t st);
 // merge of the two layers into one array ascending by t (layer 1 unpacked on the fly)

@@ -8,8 +8,9 @@
 
 namespace {
 
-constexpr int SORT_THREADS = 512;
-constexpr int SORT_IPT = 16;
+constexpr int SORT_THREADS = 512;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
+constexpr int SORT_IPT = 12;
+constexpr int SORT_MIN_BLOCKS = 2;
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 
@@ -61,157 +62,164 @@ __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const u64*
 
 // Exclusive scan over the bins of each digit, in place: hist[p][b] = number of records whose
 // digit p is smaller than b.  One block per pass.
-__global__ void sort_scan_bins_kernel(u64* hist)
+__global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64* hist)
 {
-    __shared__ u64 s[RIPS_SORT_MAX_BINS];
+    __shared__ u64 s_w[RIPS_SORT_MAX_BINS / 32];
     u64* h = hist + (size_t)blockIdx.x * RIPS_SORT_MAX_BINS;
-    for (int i = threadIdx.x; i < RIPS_SORT_MAX_BINS; i += blockDim.x) s[i] = h[i];
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        u64 run = 0;
-        for (int i = 0; i < RIPS_SORT_MAX_BINS; ++i) { u64 c = s[i]; s[i] = run; run += c; }
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u64 c = h[tid];
+    u64 incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        u64 t = __shfl_up_sync(RIPS_FULL_MASK, incl, o);
+        if (lane >= o) incl += t;
     }
+    if (lane == 31) s_w[warp] = incl;
     __syncthreads();
-    for (int i = threadIdx.x; i < RIPS_SORT_MAX_BINS; i += blockDim.x) h[i] = s[i];
+    u64 off = 0;
+#pragma unroll
+    for (int w = 0; w < RIPS_SORT_MAX_BINS / 32; ++w) off += (w < warp) ? s_w[w] : 0ull;
+    h[tid] = off + incl - c;
 }
 
 // ----------------------------------------------------------------------------------------------
-// One onesweep pass.
+// One onesweep pass.  Per tile: (1) warp-striped coalesced load; (2) rank inside each warp with
+// match.any on the digit (one MATCH per record instead of a ballot per bit) and a per-warp
+// histogram in shared memory; (3) per bin, scan over the warps, publish the tile's count for the
+// look-back at once, scan over the bins; (4) records placed in tile-sorted order in shared memory;
+// (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(SORT_THREADS) onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n,
-                                                                    int shift, int bits, const u64* __restrict__ global_base,
-                                                                    u64* status, u32* ticket)
+__global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
+onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
+                     const u64* __restrict__ global_base, u64* status, u32* ticket)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nbins = 1 << bits;
     const u32 mask = (u32)nbins - 1u;
     u64* stage = reinterpret_cast<u64*>(smem_raw);                       // [SORT_TILE]
-    u64* goff = stage + SORT_TILE;                                        // [nbins]
-    u32* whist = reinterpret_cast<u32*>(goff + nbins);                    // [SORT_WARPS][nbins]
-    u32* bin_start = whist + SORT_WARPS * nbins;                          // [nbins]
-    u32* bin_count = bin_start + nbins;                                   // [nbins] valid records per bin
+    u64* goff = stage + SORT_TILE;                                        // [MAX_BINS]
+    u32* whist = reinterpret_cast<u32*>(goff + RIPS_SORT_MAX_BINS);       // [SORT_WARPS][MAX_BINS]
+    u32* bin_start = whist + SORT_WARPS * RIPS_SORT_MAX_BINS;             // [MAX_BINS]
     __shared__ u32 s_tile;
+    __shared__ u32 s_wsum[8];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < SORT_WARPS * nbins; i += SORT_THREADS) whist[i] = 0;
+    u32* wh = whist + warp * RIPS_SORT_MAX_BINS;
+#pragma unroll
+    for (int i = lane; i < RIPS_SORT_MAX_BINS; i += 32) wh[i] = 0;
     __syncthreads();
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
     const int count = (int)min((i64)SORT_TILE, n - base);
 
-    // ---- load, warp-striped: item i of lane l of warp w is record base + w*32*IPT + i*32 + l
+    // ---- (1) load: item i of lane l of warp w is record base + w*32*IPT + i*32 + l
     u64 key[SORT_IPT];
     const i64 wbase = base + (i64)warp * (32 * SORT_IPT) + lane;
+    if (count == SORT_TILE) {
 #pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
-        i64 idx = wbase + i * 32;
-        key[i] = idx < n ? __ldg(in + idx) : ~0ull; // padding sorts last inside the tile and is never written
+        for (int i = 0; i < SORT_IPT; ++i) key[i] = __ldcs(in + wbase + i * 32);
+    } else {
+#pragma unroll
+        for (int i = 0; i < SORT_IPT; ++i) {
+            i64 idx = wbase + i * 32;
+            key[i] = idx < n ? __ldcs(in + idx) : ~0ull; // padding: last bin, last inside the tile, never written
+        }
     }
 
-    // ---- rank inside the warp: records with the same digit are found with one ballot per bit
+    // ---- (2) rank inside the warp
     u32 rank[SORT_IPT];
-    u32* wh = whist + warp * nbins;
     const u32 lt_mask = (1u << lane) - 1u;
 #pragma unroll
     for (int i = 0; i < SORT_IPT; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;
-        u32 peers = RIPS_FULL_MASK;
-        for (int b = 0; b < bits; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const u32 bal = __ballot_sync(RIPS_FULL_MASK, bit);
-            peers &= bit ? bal : ~bal;
-        }
+        const u32 peers = __match_any_sync(RIPS_FULL_MASK, d);
         const int leader = __ffs(peers) - 1;
         u32 old = 0;
-        if (lane == leader) old = wh[d];
+        if (lane == leader) { old = wh[d]; wh[d] = old + __popc(peers); }
         old = __shfl_sync(RIPS_FULL_MASK, old, leader);
-        if (lane == leader) wh[d] = old + __popc(peers);
         rank[i] = old + __popc(peers & lt_mask);
         __syncwarp();
     }
     __syncthreads();
 
-    // ---- per bin: exclusive scan over the warps; publish the tile's count for the look-back
+    // ---- (3) per bin: exclusive scan over the warps; publish; exclusive scan over the bins
     const int n_pad = SORT_TILE - count;
-    for (int b = tid; b < nbins; b += SORT_THREADS) {
+    u32 my_count = 0; // valid records of bin `tid` in this tile
+    if (tid < RIPS_SORT_MAX_BINS) {
         u32 run = 0;
+        if (tid < nbins) {
 #pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w) {
-            u32 c = whist[w * nbins + b];
-            whist[w * nbins + b] = run;
-            run += c;
-        }
-        bin_start[b] = run; // padded count for now; scanned below
-        u32 valid = (b == nbins - 1) ? run - (u32)n_pad : run;
-        bin_count[b] = valid;
-        st_volatile_u64(status + tile * nbins + b, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)valid);
-    }
-    __syncthreads();
-
-    // ---- exclusive scan over the bins (warp 0): bin_start[b] = first slot of bin b in the tile
-    if (warp == 0) {
-        const int per = nbins >> 5; // nbins is a power of two >= 32 (bits >= 5 enforced by the plan) or handled below
-        if (per >= 1) {
-            u32 sum = 0;
-            for (int j = 0; j < per; ++j) sum += bin_start[lane * per + j];
-            u32 incl = sum;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                u32 t = __shfl_up_sync(RIPS_FULL_MASK, incl, o);
-                if (lane >= o) incl += t;
-            }
-            u32 run = incl - sum;
-            for (int j = 0; j < per; ++j) {
-                u32 c = bin_start[lane * per + j];
-                bin_start[lane * per + j] = run;
+            for (int w = 0; w < SORT_WARPS; ++w) {
+                u32 c = whist[w * RIPS_SORT_MAX_BINS + tid];
+                whist[w * RIPS_SORT_MAX_BINS + tid] = run;
                 run += c;
             }
-        } else if (lane == 0) {
-            u32 run = 0;
-            for (int j = 0; j < nbins; ++j) { u32 c = bin_start[j]; bin_start[j] = run; run += c; }
+            my_count = (tid == nbins - 1) ? run - (u32)n_pad : run;
+            st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
         }
+        // block scan of `run` over the first MAX_BINS threads (8 warps)
+        u32 incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(RIPS_FULL_MASK, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) s_wsum[warp] = incl;
+        asm volatile("bar.sync 1, %0;" ::"n"(RIPS_SORT_MAX_BINS));
+        u32 woff = 0;
+#pragma unroll
+        for (int w = 0; w < RIPS_SORT_MAX_BINS / 32; ++w) woff += (w < warp) ? s_wsum[w] : 0u;
+        bin_start[tid] = woff + incl - run;
     }
     __syncthreads();
 
-    // ---- place the records in tile-sorted order in shared memory
+    // ---- (4) place the records in tile-sorted order in shared memory
 #pragma unroll
     for (int i = 0; i < SORT_IPT; ++i) {
         const u32 d = (u32)(key[i] >> shift) & mask;
         stage[bin_start[d] + wh[d] + rank[i]] = key[i];
     }
 
-    // ---- decoupled look-back, one thread per bin
-    for (int b = tid; b < nbins; b += SORT_THREADS) {
+    // ---- (5) decoupled look-back, one thread per bin
+    if (tid < nbins) {
         u64 excl = 0;
         if (tile > 0) {
             i64 t = tile - 1;
             for (;;) {
-                u64 s = ld_volatile_u64(status + t * nbins + b);
+                u64 s = ld_volatile_u64(status + t * nbins + tid);
                 u64 flag = s >> 62;
                 if (flag == 0) continue;
                 excl += s & LB_VALUE_MASK;
                 if (flag == 2) break;
                 --t;
             }
-            st_volatile_u64(status + tile * nbins + b, LB_FLAG_INC | (excl + (u64)bin_count[b]));
+            st_volatile_u64(status + tile * nbins + tid, LB_FLAG_INC | (excl + (u64)my_count));
         }
-        goff[b] = __ldg(global_base + b) + excl - (u64)bin_start[b];
+        goff[tid] = __ldg(global_base + tid) + excl - (u64)bin_start[tid];
     }
     __syncthreads();
 
-    // ---- scatter: consecutive threads write consecutive slots of a bin's run
-    for (int p = tid; p < count; p += SORT_THREADS) {
-        const u64 k = stage[p];
-        const u32 d = (u32)(k >> shift) & mask;
-        out[goff[d] + (u64)p] = k;
+    // ---- (6) scatter: consecutive threads write consecutive slots of a bin's run
+    if (count == SORT_TILE) {
+#pragma unroll
+        for (int i = 0; i < SORT_IPT; ++i) {
+            const int p = tid + i * SORT_THREADS;
+            const u64 k = stage[p];
+            out[goff[(u32)(k >> shift) & mask] + (u64)p] = k;
+        }
+    } else {
+        for (int p = tid; p < count; p += SORT_THREADS) {
+            const u64 k = stage[p];
+            out[goff[(u32)(k >> shift) & mask] + (u64)p] = k;
+        }
     }
 }
 
-size_t pass_smem_bytes(int bits)
+size_t pass_smem_bytes(int)
 {
-    size_t nbins = (size_t)1 << bits;
-    return (size_t)SORT_TILE * 8 + nbins * 8 + (size_t)SORT_WARPS * nbins * 4 + nbins * 4 * 2;
+    const size_t nb = RIPS_SORT_MAX_BINS;
+    return (size_t)SORT_TILE * 8 + nb * 8 + (size_t)SORT_WARPS * nb * 4 + nb * 4;
 }
 
 struct ScratchLayout {
@@ -240,8 +248,7 @@ SortPlan sort_make_plan(int lo_bit, int hi_bit)
     p.tile_items = SORT_TILE;
     int total = hi_bit - lo_bit;
     if (total < 1) total = 1;
-    int p8 = (total + 7) / 8, p9 = (total + 8) / 9;
-    int np = p9 < p8 ? p9 : p8;
+    int np = (total + 7) / 8; // digits of at most 8 bits (RIPS_SORT_MAX_BINS = 256)
     if (np > RIPS_SORT_MAX_PASSES) np = RIPS_SORT_MAX_PASSES; // callers never ask for more than 64 bits
     p.npasses = np;
     int basew = total / np, extra = total % np, at = lo_bit;
@@ -256,8 +263,15 @@ SortPlan sort_make_plan(int lo_bit, int hi_bit)
 
 size_t sort_scratch_bytes(i64 n, const SortPlan& plan) { return scratch_layout(n, plan).total; }
 
+u64* sort_hist_ptr(void* scratch) { return (u64*)scratch; }
+
+cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream)
+{
+    return cudaMemsetAsync(scratch, 0, (size_t)RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 8 + 256, stream);
+}
+
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream, u64** result,
-                     SortTimes* times, i64* launches)
+                     SortTimes* times, i64* launches, bool hist_ready)
 {
     *result = a;
     if (times && times->enabled) cudaEventRecord(times->ev[0], stream);
@@ -268,7 +282,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)pass_smem_bytes(9));
+                                             (int)pass_smem_bytes(8));
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(sort_histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 4);
@@ -282,7 +296,8 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     u64* status = (u64*)(sc + L.status_off);
     const i64 tiles = (n + SORT_TILE - 1) / SORT_TILE;
 
-    cudaError_t e = cudaMemsetAsync(sc, 0, L.status_off, stream);
+    cudaError_t e = cudaSuccess;
+    if (!hist_ready) e = cudaMemsetAsync(sc, 0, L.status_off, stream); // else sort_prepare_fused did it before the producer ran
     if (e != cudaSuccess) return e;
     PlanDev pd;
     pd.npasses = plan.npasses;
@@ -291,9 +306,12 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         i64 chunk = (i64)HIST_THREADS * HIST_IPT;
         i64 blocks = (n + chunk - 1) / chunk;
         if (blocks > 148 * 4) blocks = 148 * 4;
-        sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, pd, hist);
-        sort_scan_bins_kernel<<<plan.npasses, 256, 0, stream>>>(hist);
-        if (launches) *launches += 2;
+        if (!hist_ready) {
+            sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, pd, hist);
+            if (launches) *launches += 1;
+        }
+        sort_scan_bins_kernel<<<plan.npasses, RIPS_SORT_MAX_BINS, 0, stream>>>(hist);
+        if (launches) *launches += 1;
     }
     if (times && times->enabled) cudaEventRecord(times->ev[1], stream);
     u64* src = a;

@@ -5,7 +5,7 @@
 #include "common.cuh"
 
 #define RIPS_SORT_MAX_PASSES 8
-#define RIPS_SORT_MAX_BINS 512
+#define RIPS_SORT_MAX_BINS 256
 
 struct SortPlan {
     int npasses;
@@ -14,7 +14,7 @@ struct SortPlan {
     i64 tile_items;
 };
 
-// Digits covering bits [lo_bit, hi_bit): as few passes as 9-bit digits allow, widths balanced.
+// Digits covering bits [lo_bit, hi_bit): as few passes as 8-bit digits allow, widths balanced.
 SortPlan sort_make_plan(int lo_bit, int hi_bit);
 
 // Scratch the sort needs besides the ping-pong buffer, in bytes (status words, histograms, ticket).
@@ -28,5 +28,10 @@ struct SortTimes {
 // Stable LSD sort of n u64 records by the plan's digits, ascending.  `a` holds the input, `b` is the
 // ping-pong buffer; returns (via *result) which of the two holds the sorted data (a if the number
 // of passes is even).  scratch: sort_scratch_bytes(n, plan) device bytes.  launches += kernels run.
+// hist_ready: the caller zeroed the scratch head with sort_prepare_fused and a producer kernel has
+// already accumulated the raw digit counts of every pass into sort_hist_ptr(scratch)[pass][256]
+// (FusedHist in kernels.cuh); the sort then skips its own histogram read of the records.
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
-                     u64** result, SortTimes* times, i64* launches);
+                     u64** result, SortTimes* times, i64* launches, bool hist_ready = false);
+cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream);
+u64* sort_hist_ptr(void* scratch);

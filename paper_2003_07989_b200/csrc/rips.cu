@@ -54,7 +54,7 @@ struct DimState {
     // sizes
     u64 total = 0;   // C(n, d+1)
     int M = 0;       // d + 1
-    int cbits = 0, tbits = 0;
+    int cbits = 0, tbits = 0, lowbits = 0;
     // stage 1
     bool have_s1 = false;
     DevBuf colsA, colsB, s1_status, bitmap;
@@ -62,7 +62,7 @@ struct DimState {
     i64 len = 0;
     // stage 2
     bool have_s2 = false;
-    DevBuf appA, appB, non, s2_status;
+    DevBuf appA, appB, non, s2_status, nonmask;
     u64* app = nullptr; // sorted packed pair records
     i64 n_app = 0, n_non = 0;
     // reduction (second layer), sorted by t
@@ -94,6 +94,8 @@ struct rips_ctx {
     float* d_dist = nullptr;
     u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
     u32* d_K = nullptr;
+    void* d_Kf = nullptr;  // full symmetric matrix of key+1 (common.cuh)
+    int kf_u16 = 0, vbits = 1;
     float* d_values = nullptr;
     u64* d_binom = nullptr;
     u64* d_counters = nullptr; // 8 u64 scratch counters
@@ -265,7 +267,11 @@ int run_stage1(rips_ctx* c, int d)
     s.M = d + 1;
     s.total = hbinom(c, n, d + 1);
     s.cbits = bits_for(s.total ? s.total - 1 : 0);
-    if (c->key_bits + s.cbits > 64) return RIPS_EOVERFLOW;
+    s.lowbits = s.M * c->vbits;
+    if (c->key_bits + s.lowbits > 64) {
+        g_last_error = "rips_stage1: key bits + (d+1) * vertex bits exceed the 64-bit column record";
+        return RIPS_EOVERFLOW;
+    }
     // The pivots found by an earlier rips_reduce(d) depend only on the input, so they stay valid
     // (have_red) while stage 1 / stage 2 are re-run; accessors additionally require have_s2.
     s.have_s1 = s.have_s2 = false;
@@ -280,7 +286,7 @@ int run_stage1(rips_ctx* c, int d)
     s.stats = keep_stats;
     s.stats.n_candidates = (i64)s.total;
     s.stats.key_bits = c->key_bits;
-    s.stats.index_bits = s.cbits;
+    s.stats.index_bits = s.lowbits;
     s.len = 0;
     s.cols = nullptr;
     ev_record(c, s, EV_S1_BEGIN);
@@ -307,13 +313,17 @@ int run_stage1(rips_ctx* c, int d)
     const i64 tiles = stage1_tiles(s.total);
     RC(ensure(c, s.s1_status, (size_t)tiles * 8));
     Stage1Params p;
-    p.K = c->d_K;
+    p.Kf = c->d_Kf;
     p.bt = c->bt();
     p.n = (int)n;
     p.total = s.total;
+    p.tiles = tiles;
     p.thr_key = c->thr_key;
-    p.cbits = s.cbits;
+    p.vbits = c->vbits;
+    p.lowbits = s.lowbits;
     p.clear = cs;
+    p.fh.hist = nullptr;
+    p.fh.npasses = 0;
     p.status = (u64*)s.s1_status.p;
     p.ticket = c->d_tickets;
     p.counters = c->d_counters;
@@ -328,7 +338,7 @@ int run_stage1(rips_ctx* c, int d)
             CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
             CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
             p.out = nullptr;
-            CU(launch_stage1(s.M, p, c->stream));
+            CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
             c->launches += 1;
             CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
@@ -340,7 +350,17 @@ int run_stage1(rips_ctx* c, int d)
     CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
     CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
     p.out = (u64*)s.colsA.p;
-    CU(launch_stage1(s.M, p, c->stream));
+    // the digit histogram of the sort below is accumulated by the enumerate kernel itself
+    SortPlan plan = sort_make_plan(s.lowbits, s.lowbits + c->key_bits);
+    RC(ensure(c, c->sort_scratch, sort_scratch_bytes((i64)cap, plan)));
+    const bool fused = plan.npasses <= 4;
+    if (fused) {
+        CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
+        p.fh.hist = sort_hist_ptr(c->sort_scratch.p);
+        p.fh.npasses = plan.npasses;
+        for (int q = 0; q < plan.npasses; ++q) { p.fh.shift[q] = plan.shift[q]; p.fh.bits[q] = plan.bits[q]; }
+    }
+    CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
     c->launches += 1;
     ev_record(c, s, EV_S1_ENUM);
     CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
@@ -350,17 +370,15 @@ int run_stage1(rips_ctx* c, int d)
     s.stats.n_removed_by_diameter = (i64)c->h_counters[1];
     s.stats.n_cleared = (i64)c->h_counters[2];
     // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys
-    SortPlan plan = sort_make_plan(s.cbits, s.cbits + c->key_bits);
     s.stats.sort_passes = s.len > 1 ? plan.npasses : 0;
     RC(ensure(c, s.colsB, (size_t)s.len * 8));
-    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.len, plan)));
     SortTimes st;
     st.enabled = true;
     if (!s.ev_made) ev_record(c, s, EV_S1_SORTBEG);
     st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
     s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
     u64* res = nullptr;
-    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
+    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
     s.cols = res;
     ev_record(c, s, EV_S1_END);
     s.have_s1 = true;
@@ -376,7 +394,7 @@ int run_stage2(rips_ctx* c, int d)
     const i64 n = c->n;
     const u64 rows = hbinom(c, n, d + 2);
     if (rows == ~0ull) return RIPS_EOVERFLOW;
-    s.tbits = bits_for(rows ? rows - 1 : 0);
+    s.tbits = bits_for(rows); // one value more than the row indices: `rows` itself is the sentinel of non-apparent columns
     if (s.tbits + RIPS_PAIR_POS_BITS > 64 || s.tbits + c->key_bits > 64) return RIPS_EOVERFLOW;
     s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
@@ -386,48 +404,54 @@ int run_stage2(rips_ctx* c, int d)
     const i64 tiles = stage2_tiles(s.len);
     if (s.len > 0) {
         RC(ensure(c, s.appA, (size_t)s.len * 8));
-        RC(ensure(c, s.non, (size_t)s.len * 8));
-        RC(ensure(c, s.s2_status, (size_t)tiles * 16));
+        RC(ensure(c, s.nonmask, (size_t)((s.len + 31) / 32) * 4));
+        RC(ensure(c, s.s2_status, (size_t)tiles * 8));
         CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
         CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-        CU(cudaMemsetAsync(s.s2_status.p, 0, (size_t)tiles * 16, c->stream));
+        CU(cudaMemsetAsync(s.s2_status.p, 0, (size_t)tiles * 8, c->stream));
         Stage2Params p;
         p.cols = s.cols;
         p.len = s.len;
-        p.K = c->d_K;
+        p.Kf = c->d_Kf;
         p.bt = c->bt();
         p.n = (int)n;
-        p.cbits = s.cbits;
+        p.vbits = c->vbits;
+        p.lowbits = s.lowbits;
+        p.kmax = c->kmax;
         p.app_out = (u64*)s.appA.p;
-        p.non_out = (u64*)s.non.p;
-        p.status_app = (u64*)s.s2_status.p;
-        p.status_non = (u64*)s.s2_status.p + tiles;
-        p.ticket = c->d_tickets;
         p.counters = c->d_counters;
-        CU(launch_stage2(s.M, p, c->stream));
+        CU(launch_stage2(s.M, c->kf_u16, p, rows << RIPS_PAIR_POS_BITS, (u32*)s.nonmask.p, c->stream));
         c->launches += 1;
     }
     ev_record(c, s, EV_S2_APP);
     if (s.len > 0) {
-        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 8, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         s.n_app = (i64)c->h_counters[0];
-        s.n_non = (i64)c->h_counters[1];
+        s.n_non = s.len - s.n_app;
+        // a8: the non-apparent columns, in coboundary order, gathered from the bitmap
+        RC(ensure(c, s.non, (size_t)s.n_non * 8));
+        if (s.n_non > 0) {
+            CU(launch_compact_nonapparent((const u32*)s.nonmask.p, s.len, s.cols, (u64*)s.non.p, (u64*)s.s2_status.p,
+                                          c->d_tickets, c->d_counters + 1, c->stream));
+            c->launches += 1;
+        }
     }
     s.stats.n_apparent = s.n_app;
     s.stats.n_nonapparent = s.n_non;
     // ---- a9: pairs ascending by row index t
     SortPlan plan = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
-    s.stats.pair_sort_passes = s.n_app > 1 ? plan.npasses : 0;
+    s.stats.pair_sort_passes = s.len > 1 ? plan.npasses : 0;
     RC(ensure(c, s.appA, 16));
-    RC(ensure(c, s.appB, (size_t)s.n_app * 8));
-    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_app, plan)));
+    // all len records are sorted: the sentinels of the non-apparent columns sink behind the n_app pairs
+    RC(ensure(c, s.appB, (size_t)s.len * 8));
+    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.len, plan)));
     SortTimes st;
     st.enabled = true;
     st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
     s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
     u64* res = nullptr;
-    CU(sort_u64((u64*)s.appA.p, (u64*)s.appB.p, s.n_app, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
+    CU(sort_u64((u64*)s.appA.p, (u64*)s.appB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
     s.app = res;
     ev_record(c, s, EV_S2_END);
     s.have_s2 = true;
@@ -455,6 +479,14 @@ int run_reduce(rips_ctx* c, int d)
         std::vector<u64> h_non((size_t)s.n_non), h_app((size_t)s.n_app);
         CU(cudaMemcpy(h_non.data(), s.non.p, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost));
         if (s.n_app) CU(cudaMemcpy(h_app.data(), s.app, (size_t)s.n_app * 8, cudaMemcpyDeviceToHost));
+        {   // vertex-packed column records -> (key << cbits) | cidx for the host reduction (Eq. 2)
+            const u64 vmask = (1ull << c->vbits) - 1ull;
+            for (u64& r : h_non) {
+                u64 cidx = 0;
+                for (int j = 0; j < s.M; ++j) cidx += hbinom(c, (i64)((r >> (j * c->vbits)) & vmask), j + 1);
+                r = ((r >> s.lowbits) << s.cbits) | cidx;
+            }
+        }
         double t1 = now_ms();
         HostReduceIn in;
         in.n = (int)c->n;
@@ -525,7 +557,7 @@ int check_dim(rips_ctx* c, int d, int lo)
 
 void free_dim(rips_ctx* c, DimState& s)
 {
-    DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.appA, &s.appB, &s.non, &s.s2_status, &s.red_t,
+    DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.appA, &s.appB, &s.non, &s.s2_status, &s.nonmask, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
     if (s.ev_made) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(s.ev[i]);
@@ -577,8 +609,19 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
             return RIPS_EINVAL;
         }
         c->n_distinct = (u32)c->h_counters[0];
+        c->kf_u16 = c->n_distinct <= 65535u; // entries are key+1 <= n_distinct
         c->h_values.resize(c->n_distinct);
         CU(cudaMemcpy(c->h_values.data(), c->d_values, (size_t)c->n_distinct * 4, cudaMemcpyDeviceToHost));
+    }
+    {
+        const size_t kf_bytes = (((size_t)n * (size_t)n * (c->kf_u16 ? 2 : 4)) + 15) & ~(size_t)15;
+        cudaError_t e = cudaMalloc(&c->d_Kf, kf_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); g_last_error = "cudaMalloc of the full key matrix failed"; return RIPS_ENOMEM; }
+        c->dev_bytes += (i64)kf_bytes;
+        CU(cudaMemsetAsync(c->d_Kf, 0, kf_bytes, c->stream));
+        CU(launch_build_full_keys(c->d_K, (int)n, c->d_Kf, c->kf_u16, c->stream));
+        c->launches += 1;
+        c->vbits = bits_for((u64)(n - 1));
     }
     // keys are ranks in descending value order: thr_key = number of distinct values above the threshold
     u32 lo = 0, hi = c->n_distinct;
@@ -589,7 +632,6 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
     }
     c->thr_key = lo;
     c->key_bits = bits_for(c->n_distinct ? c->n_distinct - 1 : 0);
-    (void)n;
     return RIPS_OK;
 }
 
@@ -661,9 +703,9 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     int r = init_device_tables(c, dist_lower);
     if (r == RIPS_OK) {
         // the widest record of the requested dimensions must fit 64 bits
-        int cb = bits_for(hbinom(c, n, dim_max + 1) ? hbinom(c, n, dim_max + 1) - 1 : 0);
-        int tb = bits_for(hbinom(c, n, dim_max + 2) ? hbinom(c, n, dim_max + 2) - 1 : 0);
-        if (c->key_bits + cb > 64 || c->key_bits + tb > 64) r = RIPS_EOVERFLOW;
+        int lb = (dim_max + 1) * c->vbits;
+        int tb = bits_for(hbinom(c, n, dim_max + 2));
+        if ((dim_max >= 1 && c->key_bits + lb > 64) || c->key_bits + tb > 64) r = RIPS_EOVERFLOW;
     }
     if (r != RIPS_OK) { rips_free(c); return r; }
     *out = c;
@@ -681,6 +723,7 @@ void rips_free(rips_ctx* c)
     cudaFree(c->d_dist);
     cudaFree(c->d_edges);
     cudaFree(c->d_K);
+    cudaFree(c->d_Kf);
     cudaFree(c->d_values);
     cudaFree(c->d_binom);
     cudaFree(c->d_counters);
@@ -726,7 +769,7 @@ int rips_filtration(rips_ctx* c, int d, const float** diam_dev, const uint64_t**
     if (!s.has_vf) {
         RC(ensure(c, s.v_fdiam, (size_t)s.len * 4));
         RC(ensure(c, s.v_fcidx, (size_t)s.len * 8));
-        CU(launch_unpack_columns(s.cols, s.len, s.cbits, c->d_values, (float*)s.v_fdiam.p, (u64*)s.v_fcidx.p, c->stream));
+        CU(launch_unpack_columns(s.M, s.cols, s.len, c->vbits, c->bt(), c->d_values, (float*)s.v_fdiam.p, (u64*)s.v_fcidx.p, c->stream));
         c->launches += s.len > 0;
         CU(cudaStreamSynchronize(c->stream));
         s.has_vf = true;
@@ -766,7 +809,7 @@ int rips_nonapparent(rips_ctx* c, int d, const float** diam_dev, const uint64_t*
     if (!s.has_vn) {
         RC(ensure(c, s.v_ndiam, (size_t)s.n_non * 4));
         RC(ensure(c, s.v_ncidx, (size_t)s.n_non * 8));
-        CU(launch_unpack_columns((const u64*)s.non.p, s.n_non, s.cbits, c->d_values, (float*)s.v_ndiam.p,
+        CU(launch_unpack_columns(s.M, (const u64*)s.non.p, s.n_non, c->vbits, c->bt(), c->d_values, (float*)s.v_ndiam.p,
                                  (u64*)s.v_ncidx.p, c->stream));
         c->launches += s.n_non > 0;
         CU(cudaStreamSynchronize(c->stream));
