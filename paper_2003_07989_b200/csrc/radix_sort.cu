@@ -11,6 +11,7 @@ namespace {
 constexpr int SORT_THREADS = 512;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
 constexpr int SORT_IPT = 12;
 constexpr int SORT_MIN_BLOCKS = 2;
+constexpr int SORT_RANK_BATCH = 6;   // records ranked per pipelined batch (divides SORT_IPT)
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 
@@ -127,19 +128,30 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
         }
     }
 
-    // ---- (2) rank inside the warp
+    // ---- (2) rank inside the warp.  Three pipelined phases instead of one latency chain per record:
+    // all MATCHes, then one shared-memory atomic per digit group and round (the rounds of a warp
+    // reach its histogram in program order, so the value returned is the count of the earlier
+    // rounds), then the broadcasts.
     u32 rank[SORT_IPT];
     const u32 lt_mask = (1u << lane) - 1u;
 #pragma unroll
-    for (int i = 0; i < SORT_IPT; ++i) {
-        const u32 d = (u32)(key[i] >> shift) & mask;
-        const u32 peers = __match_any_sync(RIPS_FULL_MASK, d);
-        const int leader = __ffs(peers) - 1;
-        u32 old = 0;
-        if (lane == leader) { old = wh[d]; wh[d] = old + __popc(peers); }
-        old = __shfl_sync(RIPS_FULL_MASK, old, leader);
-        rank[i] = old + __popc(peers & lt_mask);
-        __syncwarp();
+    for (int h = 0; h < SORT_IPT; h += SORT_RANK_BATCH) {
+#pragma unroll
+        for (int i = h; i < h + SORT_RANK_BATCH; ++i)
+            rank[i] = __match_any_sync(RIPS_FULL_MASK, (u32)(key[i] >> shift) & mask);
+        u32 old[SORT_RANK_BATCH];
+#pragma unroll
+        for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
+            const u32 d = (u32)(key[i] >> shift) & mask;
+            old[i - h] = 0;
+            if (lane == __ffs(rank[i]) - 1) old[i - h] = atomicAdd(&wh[d], (u32)__popc(rank[i]));
+            __syncwarp();
+        }
+#pragma unroll
+        for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
+            const u32 peers = rank[i];
+            rank[i] = __shfl_sync(RIPS_FULL_MASK, old[i - h], __ffs(peers) - 1) + __popc(peers & lt_mask);
+        }
     }
     __syncthreads();
 

@@ -353,7 +353,7 @@ int run_stage1(rips_ctx* c, int d)
     // the digit histogram of the sort below is accumulated by the enumerate kernel itself
     SortPlan plan = sort_make_plan(s.lowbits, s.lowbits + c->key_bits);
     RC(ensure(c, c->sort_scratch, sort_scratch_bytes((i64)cap, plan)));
-    const bool fused = plan.npasses <= 4;
+    const bool fused = plan.npasses <= 3; // S1_MAX_FUSED digits
     if (fused) {
         CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
         p.fh.hist = sort_hist_ptr(c->sort_scratch.p);
