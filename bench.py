@@ -5,8 +5,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
 
 A "step" is one pass of the whole hot path (every row a3-a10 of DESIGN.md section 1) over one
-workload: for d = 1..dim_max: rips_stage1(d) (enumerate + diameter + threshold + clearing +
-compaction + onesweep sort), rips_stage2(d) (apparent-pair kernel + partition + pair sort), called
+workload: for d = 1..dim_max: rips_stage1(d) (fused enumerate + diameter + threshold + clearing +
+apparent-pair test, then the onesweep filtration sort), rips_stage2(d) (pair partition + the sorts
+of the small irregular / non-apparent lists), called
 through the C ABI on a context whose distance matrix, key matrix, binomial table and clearing sets
 are resident in HBM (one untimed rips_compute produced them).  `value` = candidate simplices
 (sum over d of C(n, d+1)) per second, whole job.  `e2e` = the same count divided by the time of
@@ -189,24 +190,21 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------ B200 arm
-KERNELS = {  # rips_timings field -> (kernel, launches per stage call, algorithmic bytes per launch)
-    "enumerate_ms": "stage1_kernel (a3-a5 enumerate+filter+compact)",
+KERNELS = {  # rips_timings field -> kernel
+    "enumerate_ms": "enumerate_apparent_kernel (a3-a5+a7 fused enumerate, filter, apparent test)",
     "sort_pass_ms": "onesweep_pass_kernel (a6 filtration sort)",
-    "apparent_ms": "stage2_kernel (a7-a8 apparent pairs+partition)",
-    "pair_sort_ms": "onesweep_pass_kernel (a9 pair sort)",
+    "pair_sort_ms": "onesweep_pass_kernel (a9 pair partition by cofacet vertex)",
 }
 
 
 def algorithmic_bytes(field, st):
     """HBM bytes ONE launch of the kernel must move, from rips_stats of that dimension."""
-    if field == "enumerate_ms":   # clearing bitmap read + survivors written
-        return st["n_candidates"] / 8 + RECORD_BYTES * st["n_columns"], 1
+    if field == "enumerate_ms":   # clearing bitmap read; one column record and one pair record written per slot
+        return st["n_candidates"] / 8 + 2 * RECORD_BYTES * st["n_slots"], 1
     if field == "sort_pass_ms":   # each pass reads and writes every record once
-        return 2 * RECORD_BYTES * st["n_columns"], max(1, st["sort_passes"])
-    if field == "apparent_ms":    # columns read, pairs + non-apparent columns written
-        return RECORD_BYTES * (st["n_columns"] + st["n_apparent"] + st["n_nonapparent"]), 1
+        return 2 * RECORD_BYTES * st["n_slots"], max(1, st["sort_passes"])
     if field == "pair_sort_ms":
-        return 2 * RECORD_BYTES * st["n_apparent"], max(1, st["pair_sort_passes"])
+        return 2 * RECORD_BYTES * st["n_slots"], max(1, st["pair_sort_passes"])
     raise KeyError(field)
 
 
@@ -352,9 +350,9 @@ def run_b200(args):
                 "kernels": kernels,
                 "barcode": {"end_to_end_ms": e2e_t, "first_compute_ms": first_compute_ms, **(parts or {})},
                 "stats": {str(d): {k: stats[d][k] for k in ("n_candidates", "n_columns", "n_cleared",
-                                                            "n_removed_by_diameter", "n_apparent", "n_nonapparent",
-                                                            "sort_passes", "pair_sort_passes", "key_bits",
-                                                            "index_bits")} for d in range(1, D + 1)},
+                                                            "n_removed_by_diameter", "n_apparent", "n_regular",
+                                                            "n_nonapparent", "n_slots", "sort_passes",
+                                                            "pair_sort_passes", "key_bits", "index_bits")} for d in range(1, D + 1)},
                 "device_bytes": g.device_bytes(), "parallelism": "replicas" if world > 1 else "single"}
         print(json.dumps(line))
     g.free()

@@ -64,8 +64,13 @@ typedef struct {
     int64_t n_essential;           /* columns that reduce to zero */
     int64_t n_additions;           /* column additions performed by the reduction */
     int64_t n_bars;                /* bars of non-zero length reported by rips_barcodes */
+    int64_t n_slots;               /* records the two sorts of this dimension move: C(n,d+1) when every candidate
+                                      keeps a slot (dropped ones hold a sentinel the sort sinks), n_columns when
+                                      the survivors are compacted first (thresholded inputs) */
+    int64_t n_regular;             /* apparent pairs whose cofacet vertex lies above every vertex of s (sorted by
+                                      one stable partition); the other n_apparent - n_regular are sorted in full */
     int32_t key_bits;              /* bits of the diameter rank inside a packed record */
-    int32_t index_bits;            /* bits of the combinatorial index inside a packed record */
+    int32_t index_bits;            /* bits of the vertex word inside a packed column record */
     int32_t sort_passes;           /* radix passes run by the filtration sort */
     int32_t pair_sort_passes;      /* radix passes run by the pair sort */
 } rips_stats_t;
@@ -74,12 +79,12 @@ typedef struct {
  * (host-side pieces by a host clock).  Valid after the stream has been synchronised. */
 typedef struct {
     float clear_bitmap_ms;   /* a4: clearing bitmap built from P_{d-1} */
-    float enumerate_ms;      /* a3-a5: enumerate + diameter + filter + ordered compaction */
+    float enumerate_ms;      /* a3-a5 + a7: the fused kernel (enumerate, diameter, filter, slot/compaction, apparent test) */
     float sort_hist_ms;      /* a6: digit histograms */
     float sort_pass_ms;      /* a6: all onesweep passes */
-    float apparent_ms;       /* a7-a8: apparent-pair kernel with partition */
-    float pair_hist_ms;      /* a9 */
-    float pair_sort_ms;      /* a9 */
+    float apparent_ms;       /* a8: full sorts of the two small lists (irregular pairs, non-apparent columns) */
+    float pair_hist_ms;      /* a9: bin scan (the histogram itself is accumulated by the fused kernel) */
+    float pair_sort_ms;      /* a9: stable partition of the pair slots by cofacet vertex (onesweep passes) */
     float stage1_ms;         /* whole stage 1 as enqueued (including memsets, scalar read-back) */
     float stage2_ms;         /* whole stage 2 */
     float dim0_ms;           /* d == 0 only: edge sort is part of rips_init; this is the union-find kernel */

@@ -84,25 +84,26 @@ __global__ void __launch_bounds__(RK_THREADS) rank_edges_kernel(const u64* __res
     }
 }
 
-// Kf[i*n + j] = key(i,j) + 1 for i != j, 0 on the diagonal (common.cuh)
+// Kf[i*pitch + j] = key(i,j) + 1 for i != j, 0 on the diagonal (common.cuh); the pitch makes the rows
+// of consecutive vertices fall into different shared-memory banks
 template <typename KT>
-__global__ void build_full_keys_kernel(const u32* __restrict__ K, int n, KT* __restrict__ Kf)
+__global__ void build_full_keys_kernel(const u32* __restrict__ K, int n, int pitch, KT* __restrict__ Kf)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
     if (j >= n) return;
     u32 x = 0;
     if (i != j) x = dkey(K, i, j) + 1u;
-    Kf[(size_t)i * n + j] = (KT)x;
+    Kf[(size_t)i * pitch + j] = (KT)x;
 }
 
 } // namespace
 
-cudaError_t launch_build_full_keys(const u32* K, int n, void* Kf, int kf_u16, cudaStream_t st)
+cudaError_t launch_build_full_keys(const u32* K, int n, int pitch, void* Kf, int kf_u16, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
     dim3 g((unsigned)((n + 255) / 256), (unsigned)n);
-    if (kf_u16) build_full_keys_kernel<unsigned short><<<g, 256, 0, st>>>(K, n, (unsigned short*)Kf);
-    else build_full_keys_kernel<u32><<<g, 256, 0, st>>>(K, n, (u32*)Kf);
+    if (kf_u16) build_full_keys_kernel<unsigned short><<<g, 256, 0, st>>>(K, n, pitch, (unsigned short*)Kf);
+    else build_full_keys_kernel<u32><<<g, 256, 0, st>>>(K, n, pitch, (u32*)Kf);
     return cudaGetLastError();
 }
 

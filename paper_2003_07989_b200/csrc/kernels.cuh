@@ -8,7 +8,8 @@
 //                                               (colex order = lexicographic on the decreasing vertex
 //                                               tuple, Remark 2), and spares stage 2 and
 //                                               the unpack kernels the inverse of Eq. 2.
-//   pair record     (cidx(t) << 3) | j         j = position of the added vertex v inside t
+//   regular pair    (v << tbits) | cidx(t)     v = the cofacet vertex, above every vertex of s (apparent.cuh)
+//   irregular pair  (cidx(t) << 3) | j         j = position of the added vertex v inside t
 //                                               (number of vertices of s below v); s = t minus that vertex
 //
 // Both are bijective encodings of the paper's (diameter, cidx) struct and
@@ -28,7 +29,7 @@ cudaError_t launch_rank_edges(const u64* rec_sorted, i64 E, u32* K, float* value
                               u64* n_distinct, cudaStream_t st);
 i64 rank_edges_tiles(i64 E);
 // Kf (see common.cuh) from K: n*n entries of u16 (kf_u16 != 0) or u32
-cudaError_t launch_build_full_keys(const u32* K, int n, void* Kf, int kf_u16, cudaStream_t st);
+cudaError_t launch_build_full_keys(const u32* K, int n, int pitch, void* Kf, int kf_u16, cudaStream_t st);
 
 // ------------------------------------------------------------------ dim0.cu
 struct Dim0Out {
@@ -54,54 +55,57 @@ struct FusedHist {
     int npasses;      // <= 4
     int shift[4], bits[4];
 };
+// Counters written by the fused kernel (u64 each)
+enum { S1C_KEPT = 0, S1C_OVER = 1, S1C_CLEARED = 2, S1C_REGULAR = 3, S1C_IRREGULAR = 4, S1C_NONAPP = 5 };
+
 struct Stage1Params {
-    const void* Kf;   // full key matrix (u16 or u32, see launch_stage1's kf_u16)
+    const void* Kf;   // full key matrix (u16 or u32, see launch_stage1's kf_u16), row pitch `pitch` entries
+    int pitch;
     BinomTable bt;
     int n;
     u64 total;        // C(n, d+1)
-    i64 tiles;
+    i64 tiles;        // warp chunks
     u32 thr_key;      // keep iff key >= thr_key
+    u32 sentinel_key; // key field of the column sentinel (= number of distinct keys, larger than every key)
     int vbits, lowbits;
+    int tbits;        // bits of the row index field of a regular pair record (holds C(n, d+2) as well)
     ClearSet clear;
-    u64* out;         // packed column records in increasing cidx; NULL = count only
-    u64* status;      // one word per tile, zeroed
+    int compact;      // 0: one slot per candidate, sentinels in the dropped ones (sorted away afterwards);
+                      // 1: survivors compacted in increasing index with a decoupled look-back
+    int count_only;   // 1: only counters[S1C_KEPT/OVER/CLEARED] are produced
+    u64* cols_out;    // packed column records
+    u64* pairs_out;   // same slots: regular pair record (v << tbits) | cidx(t), or the pair sentinel (n << tbits)
+    u64* irr_out;     // irregular apparent pairs (cidx(t) << 3) | j, unordered; capacity irr_cap
+    u64* non_out;     // non-apparent column records, unordered; capacity non_cap
+    u64 irr_cap, non_cap;
+    u64* status;      // one word per warp chunk, zeroed (compact mode)
     u32* ticket;      // zeroed
-    u64* counters;    // [0] kept [1] removed by diameter [2] cleared ; zeroed
-    FusedHist fh;     // histogram of the filtration sort's digits
+    u64* counters;    // S1C_*, zeroed
+    FusedHist fh_cols;   // digit histogram of the filtration sort (over every slot written to cols_out)
+    FusedHist fh_pairs;  // digit histogram of the partition of pairs_out by v
 };
 i64 stage1_tiles(u64 total);
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
-// bitmap |= bits of the given pivot rows
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, cudaStream_t st);
+// bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask
+cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st);
 
-// ------------------------------------------------------------------ stage2.cu
-struct Stage2Params {
-    const u64* cols;  // sorted packed column records
-    i64 len;
-    const void* Kf;
-    BinomTable bt;
-    int n;
-    int vbits, lowbits;
-    int kmax;         // rows of the binomial table (k = 0..kmax)
-    u64* app_out;     // one record per column (pair record or sentinel), sorted by t afterwards
-    u64* counters;    // [0] apparent ; zeroed
+// ------------------------------------------------------------------ pair store, unpack, lookup (stage2.cu)
+// The two sorted layers of apparent pairs of one dimension (the third layer, the pivots found by the
+// reduction, is a pair of plain arrays).
+struct PairLayers {
+    const u64* reg;   // (v << tbits) | cidx(t), ascending; s = t minus its top vertex v
+    i64 n_reg;
+    const u64* irr;   // (cidx(t) << 3) | j, ascending
+    i64 n_irr;
+    int tbits;
 };
-i64 stage2_tiles(i64 len);
-// app_out gets one record per column: the pair record, or `sentinel` for a non-apparent column;
-// nonmask: ceil(len/32) words, bit set <=> column is not apparent.  counters[0] += apparent.
-cudaError_t launch_stage2(int M, int kf_u16, const Stage2Params& p, u64 sentinel, u32* nonmask, cudaStream_t st);
-// ordered gather of the non-apparent columns; *counter += their number; status: stage2_tiles(len) words, zeroed
-cudaError_t launch_compact_nonapparent(const u32* nonmask, i64 len, const u64* cols, u64* non_out, u64* status, u32* ticket,
-                                       u64* counter, cudaStream_t st);
-
-// ------------------------------------------------------------------ unpack / lookup (stage2.cu)
 // packed column records -> diam[], cidx[] (M = vertices of the simplex; cidx by Eq. 2)
 cudaError_t launch_unpack_columns(int M, const u64* cols, i64 len, int vbits, BinomTable bt, const float* values,
                                   float* diam, u64* cidx, cudaStream_t st);
-// packed pair records -> t[], s[]   (M = vertices of s)
-cudaError_t launch_unpack_pairs(int M, const u64* pairs, i64 len, BinomTable bt, int n, u64* t, u64* s, cudaStream_t st);
-// merge of the two layers into one array ascending by t (layer 1 unpacked on the fly)
-cudaError_t launch_merge_pivots(int M, const u64* pairs, i64 n1, BinomTable bt, int n, const u64* red_t, const u64* red_s,
-                                i64 n2, u64* t, u64* s, cudaStream_t st);
-cudaError_t launch_pivot_lookup(int M, const u64* pairs, i64 n1, BinomTable bt, int n, const u64* red_t, const u64* red_s,
+// both apparent layers -> t[], s[] ascending by t   (M = vertices of s)
+cudaError_t launch_merge_apparent(int M, const PairLayers& L, BinomTable bt, int n, u64* t, u64* s, cudaStream_t st);
+// merge of two (t, s) arrays, both ascending by t, all t distinct
+cudaError_t launch_merge_ts(const u64* t1, const u64* s1, i64 n1, const u64* t2, const u64* s2, i64 n2, u64* t, u64* s,
+                            cudaStream_t st);
+cudaError_t launch_pivot_lookup(int M, const PairLayers& L, BinomTable bt, int n, const u64* red_t, const u64* red_s,
                                 i64 n2, const u64* query, i64 m, i64* s_out, cudaStream_t st);

@@ -36,25 +36,45 @@ struct Ctx {
             hi = lo - 1;
         }
     }
-    // first-layer lookup: s of the apparent pair whose row is t, or false
-    bool apparent_lookup(uint64_t t, uint64_t* s) const
+    // First-layer lookup: s of the apparent pair whose row is t, or false.  Evaluated directly from
+    // the definition (Definition 5) instead of searching the device array, which
+    // spares the host a copy of ~C(n-1,d+1) records: s must be the youngest facet of t -- the facet of
+    // diameter diam(t) with the smallest index (facets in increasing index = vertices removed in
+    // decreasing order, Algorithm 6) -- and t the oldest cofacet of s of that diameter (cofacets in
+    // decreasing index = added vertex decreasing, first hit).  An apparent s is a birth simplex, so it
+    // is never cleared and (s, t) is in the pair store.
+    bool apparent_lookup(uint64_t t, uint64_t* s_out) const
     {
-        int64_t lo = 0, hi = in.n_app;
-        while (lo < hi) {
-            int64_t mid = lo + (hi - lo) / 2;
-            if ((in.app[mid] >> 3) < t) lo = mid + 1;
-            else hi = mid;
-        }
-        if (lo >= in.n_app || (in.app[lo] >> 3) != t) return false;
-        int j = (int)(in.app[lo] & 7u), tv[16];
+        int tv[17];
         decode(t, M + 1, tv);
-        uint64_t r = 0;
-        for (int i = 0; i <= M; ++i) {
-            if (i < j) r += C(tv[i], i + 1);
-            else if (i > j) r += C(tv[i], i);
+        uint32_t key_t = 0xffffffffu;
+        for (int a = 1; a <= M; ++a)
+            for (int b = 0; b < a; ++b) { uint32_t k = key(tv[a], tv[b]); if (k < key_t) key_t = k; }
+        for (int drop = M; drop >= 0; --drop) {
+            int s[16], m = 0;
+            for (int i = 0; i <= M; ++i) if (i != drop) s[m++] = tv[i];
+            uint32_t key_s = 0xffffffffu;
+            for (int a = 1; a < M; ++a)
+                for (int b = 0; b < a; ++b) { uint32_t k = key(s[a], s[b]); if (k < key_s) key_s = k; }
+            if (M == 1) key_s = 0xffffffffu; // a vertex has no edge: never of the diameter of an edge t
+            if (key_s != key_t) continue;
+            // s is the youngest facet of t; is t the oldest cofacet of s with that diameter?
+            for (int v = in.n - 1; v >= 0; --v) {
+                bool member = false, ok = true;
+                for (int j = 0; j < M; ++j) {
+                    if (s[j] == v) { member = true; break; }
+                    if (key(v, s[j]) < key_s) { ok = false; break; }
+                }
+                if (member || !ok) continue;
+                if (v != tv[drop]) return false;
+                uint64_t r = 0;
+                for (int i = 0; i < M; ++i) r += C(s[i], i + 1);
+                *s_out = r;
+                return true;
+            }
+            return false;
         }
-        *s = r;
-        return true;
+        return false;
     }
     // push the coboundary of the column simplex s (cofacets with diameter <= threshold)
     template <class Heap>

@@ -14,8 +14,6 @@ struct HostReduceIn {
     const uint64_t* cols;     // packed column records of the non-apparent columns, coboundary order
     int64_t ncols;
     int cbits;
-    const uint64_t* app;      // packed pair records ascending by t (first layer of the pair store)
-    int64_t n_app;
     int tbits;                // bits of C(n, d+2) - 1
 };
 

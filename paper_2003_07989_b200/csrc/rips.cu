@@ -55,16 +55,21 @@ struct DimState {
     u64 total = 0;   // C(n, d+1)
     int M = 0;       // d + 1
     int cbits = 0, tbits = 0, lowbits = 0;
-    // stage 1
+    int compact = 0;
+    // stage 1: column records (sorted), pair slots (unsorted until stage 2), the two small lists
     bool have_s1 = false;
-    DevBuf colsA, colsB, s1_status, bitmap;
+    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch;
     u64* cols = nullptr; // sorted packed column records (points into colsA or colsB)
-    i64 len = 0;
-    // stage 2
+    i64 len = 0;         // columns
+    i64 slots = 0;       // records in the column / pair arrays (len in compact mode, else C(n,d+1) with sentinels)
+    SortPlan pair_plan;
+    bool pair_fused = false, pairs_fresh = false;
+    // stage 2: the sorted layers of the pair store
     bool have_s2 = false;
-    DevBuf appA, appB, non, s2_status, nonmask;
-    u64* app = nullptr; // sorted packed pair records
-    i64 n_app = 0, n_non = 0;
+    u64* reg = nullptr;  // regular pairs, ascending (first n_reg records of the partitioned pair slots)
+    u64* irr = nullptr;  // irregular pairs, ascending
+    u64* non = nullptr;  // non-apparent columns, coboundary order
+    i64 n_reg = 0, n_irr = 0, n_non = 0;
     // reduction (second layer), sorted by t
     bool have_red = false;
     DevBuf red_t, red_s;
@@ -95,7 +100,7 @@ struct rips_ctx {
     u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
     u32* d_K = nullptr;
     void* d_Kf = nullptr;  // full symmetric matrix of key+1 (common.cuh)
-    int kf_u16 = 0, vbits = 1;
+    int kf_u16 = 0, kf_pitch = 1, vbits = 1;
     float* d_values = nullptr;
     u64* d_binom = nullptr;
     u64* d_counters = nullptr; // 8 u64 scratch counters
@@ -242,8 +247,9 @@ int run_dim0(rips_ctx* c)
         CU(cudaMemcpy(s.red_s.p, sv.data(), (size_t)npairs * 8, cudaMemcpyHostToDevice));
     }
     s.n_red = npairs;
-    s.n_app = 0;
-    s.app = nullptr;
+    s.n_reg = s.n_irr = s.n_non = 0;
+    s.reg = s.irr = s.non = nullptr;
+    s.tbits = 1;
     s.have_s1 = s.have_s2 = s.have_red = true;
     s.stats.n_columns = n;
     s.stats.n_reduced_pivots = npairs;
@@ -254,6 +260,17 @@ int run_dim0(rips_ctx* c)
 }
 
 // ------------------------------------------------------------------------------------------ stage 1
+PairLayers layers_of(const DimState& s)
+{
+    PairLayers L;
+    L.reg = s.reg;
+    L.n_reg = s.n_reg;
+    L.irr = s.irr;
+    L.n_irr = s.n_irr;
+    L.tbits = s.tbits;
+    return L;
+}
+
 int run_stage1(rips_ctx* c, int d)
 {
     if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
@@ -266,10 +283,14 @@ int run_stage1(rips_ctx* c, int d)
     const i64 n = c->n;
     s.M = d + 1;
     s.total = hbinom(c, n, d + 1);
+    const u64 rows = hbinom(c, n, d + 2);
+    if (rows == ~0ull) return RIPS_EOVERFLOW;
     s.cbits = bits_for(s.total ? s.total - 1 : 0);
     s.lowbits = s.M * c->vbits;
-    if (c->key_bits + s.lowbits > 64) {
-        g_last_error = "rips_stage1: key bits + (d+1) * vertex bits exceed the 64-bit column record";
+    s.tbits = bits_for(rows); // one value more than the row indices, so a field of all ones is never a row
+    const int pvbits = bits_for((u64)n); // field of the cofacet vertex; n itself marks the pair sentinel
+    if (c->key_bits + s.lowbits > 64 || pvbits + s.tbits > 64 || s.tbits + RIPS_PAIR_POS_BITS > 64) {
+        g_last_error = "rips_stage1: a packed 64-bit record cannot hold this (n, dimension)";
         return RIPS_EOVERFLOW;
     }
     // The pivots found by an earlier rips_reduce(d) depend only on the input, so they stay valid
@@ -287,8 +308,9 @@ int run_stage1(rips_ctx* c, int d)
     s.stats.n_candidates = (i64)s.total;
     s.stats.key_bits = c->key_bits;
     s.stats.index_bits = s.lowbits;
-    s.len = 0;
-    s.cols = nullptr;
+    s.len = s.slots = 0;
+    s.n_reg = s.n_irr = s.n_non = 0;
+    s.cols = s.reg = s.irr = s.non = nullptr;
     ev_record(c, s, EV_S1_BEGIN);
     if (s.total == 0) {
         ev_record(c, s, EV_S1_BITMAP); ev_record(c, s, EV_S1_ENUM); ev_record(c, s, EV_S1_SORTBEG);
@@ -299,89 +321,145 @@ int run_stage1(rips_ctx* c, int d)
     // ---- a4: clearing set of dimension d-1 as a bitmap over the candidate indices
     const u64 words = (s.total + 31) / 32;
     const bool use_bitmap = words * 4 <= (8ull << 30);
-    ClearSet cs{nullptr, prev.app, prev.n_app, RIPS_PAIR_POS_BITS, (const u64*)prev.red_t.p, prev.n_red};
+    ClearSet cs{nullptr, prev.irr, prev.n_irr, RIPS_PAIR_POS_BITS, (const u64*)prev.red_t.p, prev.n_red};
     if (use_bitmap) {
         RC(ensure(c, s.bitmap, (size_t)words * 4));
         CU(cudaMemsetAsync(s.bitmap.p, 0, (size_t)words * 4, c->stream));
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.app, prev.n_app, RIPS_PAIR_POS_BITS, c->stream));
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, 0, c->stream));
-        c->launches += (prev.n_app > 0) + (prev.n_red > 0);
+        const u64 pmask = (prev.tbits >= 64) ? ~0ull : ((1ull << prev.tbits) - 1ull);
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.reg, prev.n_reg, 0, pmask, c->stream));
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.irr, prev.n_irr, RIPS_PAIR_POS_BITS, ~0ull, c->stream));
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, 0, ~0ull, c->stream));
+        c->launches += (prev.n_reg > 0) + (prev.n_irr > 0) + (prev.n_red > 0);
         cs.bitmap = (const u32*)s.bitmap.p;
+    } else if (prev.n_reg > 0) {
+        g_last_error = "rips_stage1: candidate space too large for the clearing bitmap";
+        return RIPS_ENOMEM;
     }
     ev_record(c, s, EV_S1_BITMAP);
-    // ---- a3-a5
+
+    // ---- a3-a5 + a7: the fused kernel
+    // mode: without a threshold at least (n-d-1)/n of the candidates survive (only clearing drops
+    // any), so every candidate keeps its slot; with one, estimate the surviving share from the share
+    // q of admissible edges (q^(edges of the simplex)) and compact when most are dropped
+    const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
+    s.compact = (c->thr_key != 0 && std::pow(q, (double)(s.M * (s.M - 1) / 2)) < 0.5) ? 1 : 0;
     const i64 tiles = stage1_tiles(s.total);
-    RC(ensure(c, s.s1_status, (size_t)tiles * 8));
     Stage1Params p;
     p.Kf = c->d_Kf;
+    p.pitch = c->kf_pitch;
     p.bt = c->bt();
     p.n = (int)n;
     p.total = s.total;
     p.tiles = tiles;
     p.thr_key = c->thr_key;
+    p.sentinel_key = c->n_distinct;
     p.vbits = c->vbits;
     p.lowbits = s.lowbits;
+    p.tbits = s.tbits;
     p.clear = cs;
-    p.fh.hist = nullptr;
-    p.fh.npasses = 0;
-    p.status = (u64*)s.s1_status.p;
+    p.compact = s.compact;
+    p.count_only = 0;
+    p.cols_out = p.pairs_out = p.irr_out = p.non_out = nullptr;
+    p.irr_cap = p.non_cap = 0;
+    p.status = nullptr;
     p.ticket = c->d_tickets;
     p.counters = c->d_counters;
-    u64 cap;
-    if (c->thr_key == 0) {
-        cap = s.total - (u64)(prev.n_app + prev.n_red); // every pivot row of d-1 is a candidate below the threshold
-    } else {
+    p.fh_cols.hist = p.fh_pairs.hist = nullptr;
+    p.fh_cols.npasses = p.fh_pairs.npasses = 0;
+
+    u64 cap = s.total; // slots of the two record arrays
+    if (s.compact) {
         size_t free_b = 0, total_b = 0;
         cudaMemGetInfo(&free_b, &total_b);
-        cap = s.total;
-        if (s.total * 8 > free_b / 8 && s.colsA.cap < s.total * 8) { // count first, then allocate exactly
+        if (s.total * 8 > free_b / 16 && s.colsA.cap < s.total * 8) { // count first, then allocate exactly
             CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
             CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-            p.out = nullptr;
+            p.count_only = 1;
             CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
             c->launches += 1;
-            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
+            p.count_only = 0;
+            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
-            cap = c->h_counters[0];
+            cap = c->h_counters[S1C_KEPT];
         }
+        RC(ensure(c, s.s1_status, (size_t)tiles * 8));
+        p.status = (u64*)s.s1_status.p;
     }
     RC(ensure(c, s.colsA, (size_t)cap * 8));
-    CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
-    CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-    CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
-    p.out = (u64*)s.colsA.p;
-    // the digit histogram of the sort below is accumulated by the enumerate kernel itself
+    RC(ensure(c, s.pairsA, (size_t)cap * 8));
+    p.cols_out = (u64*)s.colsA.p;
+    p.pairs_out = (u64*)s.pairsA.p;
+    // digit histograms of the two sorts are accumulated by the kernel itself
     SortPlan plan = sort_make_plan(s.lowbits, s.lowbits + c->key_bits);
+    s.pair_plan = sort_make_plan(s.tbits, s.tbits + pvbits);
     RC(ensure(c, c->sort_scratch, sort_scratch_bytes((i64)cap, plan)));
-    const bool fused = plan.npasses <= 3; // S1_MAX_FUSED digits
-    if (fused) {
-        CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
-        p.fh.hist = sort_hist_ptr(c->sort_scratch.p);
-        p.fh.npasses = plan.npasses;
-        for (int q = 0; q < plan.npasses; ++q) { p.fh.shift[q] = plan.shift[q]; p.fh.bits[q] = plan.bits[q]; }
+    RC(ensure(c, s.pair_scratch, sort_scratch_bytes((i64)cap, s.pair_plan)));
+    const bool fused = plan.npasses <= 3;           // S1_MAX_FUSED digits
+    s.pair_fused = s.pair_plan.npasses <= 2;        // S1_MAX_FUSED_P digits
+    u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 64));
+    u64 non_cap = std::max<u64>(s.nonA.cap / 8, std::max<u64>(4096, cap / 16));
+    for (int attempt = 0;; ++attempt) {
+        RC(ensure(c, s.irrA, (size_t)irr_cap * 8));
+        RC(ensure(c, s.nonA, (size_t)non_cap * 8));
+        p.irr_out = (u64*)s.irrA.p;
+        p.non_out = (u64*)s.nonA.p;
+        p.irr_cap = irr_cap;
+        p.non_cap = non_cap;
+        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+        CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+        if (s.compact) CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
+        if (fused) {
+            CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
+            p.fh_cols.hist = sort_hist_ptr(c->sort_scratch.p);
+            p.fh_cols.npasses = plan.npasses;
+            for (int r = 0; r < plan.npasses; ++r) { p.fh_cols.shift[r] = plan.shift[r]; p.fh_cols.bits[r] = plan.bits[r]; }
+        }
+        if (s.pair_fused) {
+            CU(sort_prepare_fused(s.pair_scratch.p, c->stream));
+            p.fh_pairs.hist = sort_hist_ptr(s.pair_scratch.p);
+            p.fh_pairs.npasses = s.pair_plan.npasses;
+            for (int r = 0; r < s.pair_plan.npasses; ++r) {
+                p.fh_pairs.shift[r] = s.pair_plan.shift[r];
+                p.fh_pairs.bits[r] = s.pair_plan.bits[r];
+            }
+        }
+        CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
+        c->launches += 1;
+        ev_record(c, s, EV_S1_ENUM);
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        const u64 ni = c->h_counters[S1C_IRREGULAR], nn = c->h_counters[S1C_NONAPP];
+        if (ni <= irr_cap && nn <= non_cap) break;
+        if (attempt >= 1) { g_last_error = "rips_stage1: list capacities still too small on the second attempt"; return RIPS_ECUDA; }
+        irr_cap = std::max(irr_cap, ni); // rare: more irregular pairs / non-apparent columns than provisioned; run again
+        non_cap = std::max(non_cap, nn);
     }
-    CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
-    c->launches += 1;
-    ev_record(c, s, EV_S1_ENUM);
-    CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    s.len = (i64)c->h_counters[0];
+    s.len = (i64)c->h_counters[S1C_KEPT];
+    s.slots = s.compact ? s.len : (i64)s.total;
+    s.n_reg = (i64)c->h_counters[S1C_REGULAR];
+    s.n_irr = (i64)c->h_counters[S1C_IRREGULAR];
+    s.n_non = (i64)c->h_counters[S1C_NONAPP];
     s.stats.n_columns = s.len;
-    s.stats.n_removed_by_diameter = (i64)c->h_counters[1];
-    s.stats.n_cleared = (i64)c->h_counters[2];
-    // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys
-    s.stats.sort_passes = s.len > 1 ? plan.npasses : 0;
-    RC(ensure(c, s.colsB, (size_t)s.len * 8));
+    s.stats.n_removed_by_diameter = (i64)c->h_counters[S1C_OVER];
+    s.stats.n_cleared = (i64)c->h_counters[S1C_CLEARED];
+    s.stats.n_apparent = s.n_reg + s.n_irr;
+    s.stats.n_nonapparent = s.n_non;
+    s.stats.n_slots = s.slots;
+    s.stats.n_regular = s.n_reg;
+    // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys,
+    // and the sentinels of the dropped candidates (largest key) end up behind the len columns
+    s.stats.sort_passes = s.slots > 1 ? plan.npasses : 0;
+    RC(ensure(c, s.colsB, (size_t)s.slots * 8));
     SortTimes st;
     st.enabled = true;
-    if (!s.ev_made) ev_record(c, s, EV_S1_SORTBEG);
     st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
     s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
     u64* res = nullptr;
-    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
+    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.slots, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
     s.cols = res;
     ev_record(c, s, EV_S1_END);
     s.have_s1 = true;
+    s.pairs_fresh = true;
     return RIPS_OK;
 }
 
@@ -391,69 +469,43 @@ int run_stage2(rips_ctx* c, int d)
     if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s1) { g_last_error = "rips_stage2: rips_stage1 has not run for this dimension"; return RIPS_EINVAL; }
-    const i64 n = c->n;
-    const u64 rows = hbinom(c, n, d + 2);
-    if (rows == ~0ull) return RIPS_EOVERFLOW;
-    s.tbits = bits_for(rows); // one value more than the row indices: `rows` itself is the sentinel of non-apparent columns
-    if (s.tbits + RIPS_PAIR_POS_BITS > 64 || s.tbits + c->key_bits > 64) return RIPS_EOVERFLOW;
+    if (s.have_s2 && !s.pairs_fresh) return RIPS_OK; // nothing new to partition: the pair store is current
     s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
-    s.n_app = s.n_non = 0;
-    s.app = nullptr;
     ev_record(c, s, EV_S2_BEGIN);
-    const i64 tiles = stage2_tiles(s.len);
-    if (s.len > 0) {
-        RC(ensure(c, s.appA, (size_t)s.len * 8));
-        RC(ensure(c, s.nonmask, (size_t)((s.len + 31) / 32) * 4));
-        RC(ensure(c, s.s2_status, (size_t)tiles * 8));
-        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
-        CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-        CU(cudaMemsetAsync(s.s2_status.p, 0, (size_t)tiles * 8, c->stream));
-        Stage2Params p;
-        p.cols = s.cols;
-        p.len = s.len;
-        p.Kf = c->d_Kf;
-        p.bt = c->bt();
-        p.n = (int)n;
-        p.vbits = c->vbits;
-        p.lowbits = s.lowbits;
-        p.kmax = c->kmax;
-        p.app_out = (u64*)s.appA.p;
-        p.counters = c->d_counters;
-        CU(launch_stage2(s.M, c->kf_u16, p, rows << RIPS_PAIR_POS_BITS, (u32*)s.nonmask.p, c->stream));
-        c->launches += 1;
+    // ---- a8: the two small out-of-order lists: irregular pairs by cidx(t), non-apparent columns by
+    // (key, vertices), which is the coboundary order
+    {
+        SortPlan pi = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
+        RC(ensure(c, s.irrA, 16));
+        RC(ensure(c, s.irrB, (size_t)s.n_irr * 8));
+        RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_irr, pi)));
+        u64* res = nullptr;
+        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, s.n_irr, pi, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        s.irr = res;
+        SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
+        RC(ensure(c, s.nonA, 16));
+        RC(ensure(c, s.nonB, (size_t)s.n_non * 8));
+        RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_non, pn)));
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        s.non = res;
     }
     ev_record(c, s, EV_S2_APP);
-    if (s.len > 0) {
-        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 8, cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        s.n_app = (i64)c->h_counters[0];
-        s.n_non = s.len - s.n_app;
-        // a8: the non-apparent columns, in coboundary order, gathered from the bitmap
-        RC(ensure(c, s.non, (size_t)s.n_non * 8));
-        if (s.n_non > 0) {
-            CU(launch_compact_nonapparent((const u32*)s.nonmask.p, s.len, s.cols, (u64*)s.non.p, (u64*)s.s2_status.p,
-                                          c->d_tickets, c->d_counters + 1, c->stream));
-            c->launches += 1;
-        }
-    }
-    s.stats.n_apparent = s.n_app;
-    s.stats.n_nonapparent = s.n_non;
-    // ---- a9: pairs ascending by row index t
-    SortPlan plan = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
-    s.stats.pair_sort_passes = s.len > 1 ? plan.npasses : 0;
-    RC(ensure(c, s.appA, 16));
-    // all len records are sorted: the sentinels of the non-apparent columns sink behind the n_app pairs
-    RC(ensure(c, s.appB, (size_t)s.len * 8));
-    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.len, plan)));
+    // ---- a9: stable partition of the pair slots by the cofacet vertex v: the regular pairs come out
+    // ascending by cidx(t), the sentinels (v = n) behind them
+    s.stats.pair_sort_passes = s.slots > 1 ? s.pair_plan.npasses : 0;
+    RC(ensure(c, s.pairsA, 16));
+    RC(ensure(c, s.pairsB, (size_t)s.slots * 8));
     SortTimes st;
     st.enabled = true;
     st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
     s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
     u64* res = nullptr;
-    CU(sort_u64((u64*)s.appA.p, (u64*)s.appB.p, s.len, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches));
-    s.app = res;
+    CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, c->stream, &res, &st,
+                &c->launches, s.pair_fused));
+    s.reg = res;
     ev_record(c, s, EV_S2_END);
+    s.pairs_fresh = false;
     s.have_s2 = true;
     return RIPS_OK;
 }
@@ -476,9 +528,8 @@ int run_reduce(rips_ctx* c, int d)
             c->h_K.resize((size_t)c->E);
             CU(cudaMemcpy(c->h_K.data(), c->d_K, (size_t)c->E * 4, cudaMemcpyDeviceToHost));
         }
-        std::vector<u64> h_non((size_t)s.n_non), h_app((size_t)s.n_app);
-        CU(cudaMemcpy(h_non.data(), s.non.p, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost));
-        if (s.n_app) CU(cudaMemcpy(h_app.data(), s.app, (size_t)s.n_app * 8, cudaMemcpyDeviceToHost));
+        std::vector<u64> h_non((size_t)s.n_non);
+        CU(cudaMemcpy(h_non.data(), s.non, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost));
         {   // vertex-packed column records -> (key << cbits) | cidx for the host reduction (Eq. 2)
             const u64 vmask = (1ull << c->vbits) - 1ull;
             for (u64& r : h_non) {
@@ -498,8 +549,6 @@ int run_reduce(rips_ctx* c, int d)
         in.cols = h_non.data();
         in.ncols = s.n_non;
         in.cbits = s.cbits;
-        in.app = h_app.data();
-        in.n_app = s.n_app;
         in.tbits = s.tbits;
         host_reduce_columns(in, out);
         double t2 = now_ms();
@@ -557,7 +606,8 @@ int check_dim(rips_ctx* c, int d, int lo)
 
 void free_dim(rips_ctx* c, DimState& s)
 {
-    DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.appA, &s.appB, &s.non, &s.s2_status, &s.nonmask, &s.red_t,
+    DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.pairsA, &s.pairsB, &s.irrA, &s.irrB, &s.nonA, &s.nonB,
+                     &s.pair_scratch, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
     if (s.ev_made) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(s.ev[i]);
@@ -614,12 +664,18 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         CU(cudaMemcpy(c->h_values.data(), c->d_values, (size_t)c->n_distinct * 4, cudaMemcpyDeviceToHost));
     }
     {
-        const size_t kf_bytes = (((size_t)n * (size_t)n * (c->kf_u16 ? 2 : 4)) + 15) & ~(size_t)15;
+        // row pitch: an odd number of 32-bit words, so the rows of consecutive vertices start in
+        // different shared-memory banks (lanes of the fused kernel read column v of rows x, x+1, ...)
+        int pitch = (int)n;
+        if (c->kf_u16) { while ((pitch & 3) != 2) ++pitch; }
+        else if ((pitch & 1) == 0) ++pitch;
+        c->kf_pitch = pitch;
+        const size_t kf_bytes = (((size_t)n * (size_t)pitch * (c->kf_u16 ? 2 : 4)) + 15) & ~(size_t)15;
         cudaError_t e = cudaMalloc(&c->d_Kf, kf_bytes);
         if (e != cudaSuccess) { cudaGetLastError(); g_last_error = "cudaMalloc of the full key matrix failed"; return RIPS_ENOMEM; }
         c->dev_bytes += (i64)kf_bytes;
         CU(cudaMemsetAsync(c->d_Kf, 0, kf_bytes, c->stream));
-        CU(launch_build_full_keys(c->d_K, (int)n, c->d_Kf, c->kf_u16, c->stream));
+        CU(launch_build_full_keys(c->d_K, (int)n, pitch, c->d_Kf, c->kf_u16, c->stream));
         c->launches += 1;
         c->vbits = bits_for((u64)(n - 1));
     }
@@ -631,7 +687,7 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         else hi = mid;
     }
     c->thr_key = lo;
-    c->key_bits = bits_for(c->n_distinct ? c->n_distinct - 1 : 0);
+    c->key_bits = bits_for(c->n_distinct); // the value n_distinct itself is the key of the column sentinel
     return RIPS_OK;
 }
 
@@ -705,7 +761,8 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
         // the widest record of the requested dimensions must fit 64 bits
         int lb = (dim_max + 1) * c->vbits;
         int tb = bits_for(hbinom(c, n, dim_max + 2));
-        if ((dim_max >= 1 && c->key_bits + lb > 64) || c->key_bits + tb > 64) r = RIPS_EOVERFLOW;
+        if ((dim_max >= 1 && c->key_bits + lb > 64) || c->key_bits + tb > 64 || bits_for((u64)n) + tb > 64)
+            r = RIPS_EOVERFLOW;
     }
     if (r != RIPS_OK) { rips_free(c); return r; }
     *out = c;
@@ -787,16 +844,16 @@ int rips_apparent_pairs(rips_ctx* c, int d, const uint64_t** t_dev, const uint64
     DimState& s = c->dims[d];
     if (!s.have_s2) return RIPS_EINVAL;
     if (!s.has_va) {
-        RC(ensure(c, s.v_at, (size_t)s.n_app * 8));
-        RC(ensure(c, s.v_as, (size_t)s.n_app * 8));
-        CU(launch_unpack_pairs(s.M, s.app, s.n_app, c->bt(), (int)c->n, (u64*)s.v_at.p, (u64*)s.v_as.p, c->stream));
-        c->launches += s.n_app > 0;
+        RC(ensure(c, s.v_at, (size_t)(s.n_reg + s.n_irr) * 8));
+        RC(ensure(c, s.v_as, (size_t)(s.n_reg + s.n_irr) * 8));
+        CU(launch_merge_apparent(s.M, layers_of(s), c->bt(), (int)c->n, (u64*)s.v_at.p, (u64*)s.v_as.p, c->stream));
+        c->launches += (s.n_reg + s.n_irr) > 0;
         CU(cudaStreamSynchronize(c->stream));
         s.has_va = true;
     }
     *t_dev = (const u64*)s.v_at.p;
     *s_dev = (const u64*)s.v_as.p;
-    *n_app = s.n_app;
+    *n_app = s.n_reg + s.n_irr;
     return RIPS_OK;
 }
 
@@ -809,7 +866,7 @@ int rips_nonapparent(rips_ctx* c, int d, const float** diam_dev, const uint64_t*
     if (!s.has_vn) {
         RC(ensure(c, s.v_ndiam, (size_t)s.n_non * 4));
         RC(ensure(c, s.v_ncidx, (size_t)s.n_non * 8));
-        CU(launch_unpack_columns(s.M, (const u64*)s.non.p, s.n_non, c->vbits, c->bt(), c->d_values, (float*)s.v_ndiam.p,
+        CU(launch_unpack_columns(s.M, s.non, s.n_non, c->vbits, c->bt(), c->d_values, (float*)s.v_ndiam.p,
                                  (u64*)s.v_ncidx.p, c->stream));
         c->launches += s.n_non > 0;
         CU(cudaStreamSynchronize(c->stream));
@@ -827,12 +884,19 @@ int rips_pivots(rips_ctx* c, int d, const uint64_t** t_dev, const uint64_t** s_d
     if (!t_dev || !s_dev || !n_piv) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_red || !s.have_s2) return RIPS_EINVAL;
-    const i64 np = s.n_app + s.n_red;
+    const i64 na = s.n_reg + s.n_irr, np = na + s.n_red;
     if (!s.has_vp) {
+        if (!s.has_va) { // the apparent layers as (t, s) arrays first
+            RC(ensure(c, s.v_at, (size_t)na * 8));
+            RC(ensure(c, s.v_as, (size_t)na * 8));
+            CU(launch_merge_apparent(s.M, layers_of(s), c->bt(), (int)c->n, (u64*)s.v_at.p, (u64*)s.v_as.p, c->stream));
+            c->launches += na > 0;
+            s.has_va = true;
+        }
         RC(ensure(c, s.v_pt, (size_t)np * 8));
         RC(ensure(c, s.v_ps, (size_t)np * 8));
-        CU(launch_merge_pivots(s.M, s.app, s.n_app, c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
-                               s.n_red, (u64*)s.v_pt.p, (u64*)s.v_ps.p, c->stream));
+        CU(launch_merge_ts((const u64*)s.v_at.p, (const u64*)s.v_as.p, na, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
+                           s.n_red, (u64*)s.v_pt.p, (u64*)s.v_ps.p, c->stream));
         c->launches += np > 0;
         CU(cudaStreamSynchronize(c->stream));
         s.has_vp = true;
@@ -849,7 +913,7 @@ int rips_pivot_lookup(rips_ctx* c, int d, const uint64_t* t_query_dev, int64_t m
     if (m < 0 || (m > 0 && (!t_query_dev || !s_out_dev))) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) return RIPS_EINVAL;
-    CU(launch_pivot_lookup(s.M, s.app, s.n_app, c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
+    CU(launch_pivot_lookup(s.M, layers_of(s), c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
                            s.have_red ? s.n_red : 0, t_query_dev, m, s_out_dev, c->stream));
     c->launches += m > 0;
     CU(cudaStreamSynchronize(c->stream));

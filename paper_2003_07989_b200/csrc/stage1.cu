@@ -1,20 +1,38 @@
-// stage1.cu -- steps a3-a5: enumerate + diameter + threshold + clearing + ordered compaction.
-// Algorithm 7 "filter-columns-kernel" and the count of Algorithm 8, redesigned:
-// the paper launches one thread per candidate with a binary-search decode and leaves
-// sentinels in place for the sort to sink.  Here a warp walks a chunk of consecutive indices row by
-// row (see the kernel), decodes once per chunk (closed-form estimate + exact fix-up), survivors
-// are compacted in increasing index with a decoupled look-back, so only survivors are ever written
-// or sorted, and the digit histogram of the sort that follows is accumulated on the way out, which
-// spares that sort its own read of the records.
+// stage1.cu -- the fused hot kernel: steps a3-a5 (enumerate + diameter + threshold + clearing +
+// compaction, Algorithms 7-8) and a7 (the apparent-pair test, Algorithm 3 /
+// Lemma 7) in one pass over the candidate index space.
+//
+// Redesign against the paper (which launches one thread per candidate with a binary-search decode,
+// PAPER.md:359, :605, sorts, and only then runs one thread per sorted column):
+//   * a warp owns a chunk of consecutive combinatorial indices and walks it row by row: a row fixes
+//     the vertices v[M-1] > ... > v[1] (warp-uniform) and the lanes take consecutive lowest
+//     vertices v[0].  What depends only on the row -- the keys among the upper vertices, and
+//     U[v] = min_j key(v_j, v) for the 32 highest v, the part of every cofacet test the row shares --
+//     is computed once per row; each lane adds one read of its own row of Kf.
+//   * the apparent test of a column is independent of the column order (Corollary 8, PAPER.md:
+//     297-299; Prop. 10), so it runs here, where the column's vertices and key are
+//     in registers, in increasing cidx.  In that order the regular pairs (apparent.cuh) need a single
+//     stable partition by v to be sorted by cidx(t), instead of a full radix sort of 31+ bits.
+//   * lanes whose scan leaves the 32-vertex window, or stops below the top vertex of s (the facet
+//     test is then needed), go to a small per-warp queue that the warp drains cooperatively, 32
+//     cofacet vertices per step: the long tail of the scan never serialises a warp.
+//   * without a threshold (>= 98 % survive) every candidate keeps its slot and dropped ones get a
+//     sentinel that the sort sinks (the paper's device): no compaction, fully
+//     coalesced stores.  With a threshold survivors are compacted in increasing index with a
+//     warp-level decoupled look-back.
+//   * the digit histograms of the two sorts that follow are accumulated on the way out.
+#include "apparent.cuh"
 #include "kernels.cuh"
 
 namespace {
 
-constexpr int S1_THREADS = 256;
+constexpr int S1_THREADS = 512;
 constexpr int S1_WARPS = S1_THREADS / 32;
-constexpr int S1_CHUNK = 512;                 // candidates per warp chunk = unit of the look-back chain
-constexpr int S1_BLOCKS_PER_SM = 6;
-constexpr int S1_MAX_FUSED = 3;               // digits of the following sort histogrammed on the way out
+constexpr int S1_CHUNK = 512;          // candidates per warp chunk = unit of the look-back chain
+constexpr int S1_QCAP = 64;            // queue entries per warp (drained when fewer than 32 are free)
+constexpr int S1_MAX_FUSED = 3;        // digits of the filtration sort histogrammed on the way out
+constexpr int S1_MAX_FUSED_P = 2;      // digits of the pair partition
+constexpr size_t S1_KF_SMEM_LIMIT = 80 * 1024;   // two blocks per SM with the queues beside it
 
 __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int shift, u64 x)
 {
@@ -27,39 +45,152 @@ __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int 
     return lo < n && (__ldg(a + lo) >> shift) == x;
 }
 
-// A warp owns a chunk of S1_CHUNK consecutive combinatorial indices and walks it row by row: a
-// row fixes the vertices v[M-1] > ... > v[1] (warp-uniform: their mutual keys, the row pointers
-// into Kf and the upper part of the record are computed once per row) and the lanes take
-// consecutive lowest vertices v[0], so every read of the key matrix is coalesced and no lane
-// ever carries on its own.  The warp's survivors are staged in shared memory in index order and
-// written out after a warp-level decoupled look-back over the chunks (no block-wide barrier).
-template <int M, typename KT>
-__global__ void __launch_bounds__(S1_THREADS) stage1_kernel(const Stage1Params p)
+struct WarpQueue {
+    u64* rec;   // column record
+    u64* idx;   // cidx(s)
+    int* vs;    // first cofacet vertex still to test
+    u32* slot;  // compact mode: slot in the warp's staging arrays
+};
+
+// append `val` to a global list with capacity `cap`; the counter keeps counting past the capacity
+__device__ __forceinline__ void list_append(u64* list, u64 cap, u64* counter, u64 val)
 {
-    __shared__ u64 stage[S1_WARPS][S1_CHUNK];
-    __shared__ u32 s_hist[S1_MAX_FUSED][256];
+    u64 pos = atomicAdd((unsigned long long*)counter, 1ull);
+    if (pos < cap) list[pos] = val;
+}
+
+
+// shared-memory digit histograms of one block
+struct BlockHists {
+    u32 (*cols)[256];   // [S1_MAX_FUSED][256]
+    u32 (*pairs)[256];  // [S1_MAX_FUSED_P][256]
+    int ncols, npairs;
+    int csh[S1_MAX_FUSED];
+    u32 cmk[S1_MAX_FUSED];
+    int psh[S1_MAX_FUSED_P];
+    u32 pmk[S1_MAX_FUSED_P];
+};
+
+// Warp-cooperative drain of the queue: per entry, 32 cofacet vertices are tested per step (lane l
+// takes v = base - l, so the reads of Kf are consecutive), then the warp-uniform classification:
+// regular pair, irregular pair (facet test), or non-apparent column.
+template <int M, typename KT>
+__device__ __forceinline__ void drain_queue(const Stage1Params& p, const KT* Kf, const WarpQueue& q, int qcount, int lane,
+                                            u64* stage_pairs, const BlockHists& H, u64 psentinel, u32& n_reg)
+{
+    __syncwarp();
+    for (int e = 0; e < qcount; ++e) {
+        const u64 rec = q.rec[e];
+        const u64 idx = q.idx[e];
+        const int vs = q.vs[e];
+        const u32 key1 = (u32)(rec >> p.lowbits) + 1u;
+        int s[M];
+        unpack_vertices<M>(rec, p.vbits, s);
+        int fv = -1;
+        for (int base = vs; base >= 0; base -= 32) {
+            const int vv = base - lane;
+            bool ok = false;
+            if (vv >= 0) {
+                u32 m = 0xffffffffu;
+#pragma unroll
+                for (int j = 0; j < M; ++j) m = min(m, (u32)Kf[s[j] * p.pitch + vv]);
+                ok = m >= key1;
+            }
+            const u32 b = __ballot_sync(RIPS_FULL_MASK, ok);
+            if (b) { fv = base - (__ffs(b) - 1); break; }
+        }
+        u64 prec = psentinel;
+        bool is_non = true;
+        u64 irr = 0;
+        if (fv >= 0) {
+            int fseg = 0;
+#pragma unroll
+            for (int j = 0; j < M; ++j) fseg += (s[j] < fv) ? 1 : 0;
+            if (fseg == M) {
+                prec = ((u64)(u32)fv << p.tbits) | (idx + p.bt(fv, M + 1));
+                is_non = false;
+                if (lane == 0) ++n_reg;
+            } else if (s_is_youngest_facet<M, KT>(Kf, p.pitch, s, key1, fv, fseg)) {
+                irr = (cofacet_index<M>(p.bt, s, fv, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
+                is_non = false;
+                if (lane == 0) list_append(p.irr_out, p.irr_cap, p.counters + S1C_IRREGULAR, irr);
+            }
+        }
+        if (lane == 0) {
+            if (is_non) list_append(p.non_out, p.non_cap, p.counters + S1C_NONAPP, rec);
+            if (p.compact) stage_pairs[q.slot[e]] = prec;
+            else __stcs(p.pairs_out + idx, prec);
+#pragma unroll
+            for (int r = 0; r < S1_MAX_FUSED_P; ++r)
+                if (r < H.npairs) atomicAdd(&H.pairs[r][(u32)(prec >> H.psh[r]) & H.pmk[r]], 1u);
+        }
+    }
+    __syncwarp();
+}
+
+template <int M, typename KT>
+__global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const Stage1Params p, int k_in_smem)
+{
+    extern __shared__ __align__(16) unsigned char smem1[];
+    __shared__ u32 s_hist_cols[S1_MAX_FUSED][256];
+    __shared__ u32 s_hist_pairs[S1_MAX_FUSED_P][256];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const KT* __restrict__ Kf = reinterpret_cast<const KT*>(p.Kf);
-    const int n = p.n, vbits = p.vbits, lowbits = p.lowbits;
+    const int n = p.n, pitch = p.pitch, vbits = p.vbits, lowbits = p.lowbits;
     const u32 lt_mask = (1u << lane) - 1u;
     const u32 thr1 = p.thr_key + 1u; // keys in Kf are shifted by one
-    const bool write = p.out != nullptr;
-    const int nfused = (write && p.fh.hist != nullptr) ? p.fh.npasses : 0;
-    int fsh[S1_MAX_FUSED];
-    u32 fmk[S1_MAX_FUSED];
+    const bool compact = p.compact != 0, count_only = p.count_only != 0;
+    const u64 csentinel = (u64)p.sentinel_key << lowbits;
+    const u64 psentinel = (u64)(u32)n << p.tbits;
+
+    // ---- shared memory carve-up: [Kf] [queues] [staging (compact mode)]
+    size_t off_b = 0;
+    const KT* Kf = reinterpret_cast<const KT*>(p.Kf);
+    if (k_in_smem) {
+        const int cnt16 = (int)(((size_t)n * pitch * sizeof(KT) + 15) / 16); // the buffer is padded to 16 bytes
+        uint4* dst = reinterpret_cast<uint4*>(smem1);
+        const uint4* src = reinterpret_cast<const uint4*>(p.Kf);
+        for (int i = tid; i < cnt16; i += S1_THREADS) dst[i] = __ldg(src + i);
+        Kf = reinterpret_cast<const KT*>(smem1);
+        off_b = (size_t)cnt16 * 16;
+    }
+    WarpQueue q;
+    {
+        unsigned char* qb = smem1 + off_b + (size_t)warp * (S1_QCAP * 24);
+        q.rec = reinterpret_cast<u64*>(qb);
+        q.idx = q.rec + S1_QCAP;
+        q.vs = reinterpret_cast<int*>(q.idx + S1_QCAP);
+        q.slot = reinterpret_cast<u32*>(q.vs + S1_QCAP);
+        off_b += (size_t)S1_WARPS * (S1_QCAP * 24);
+    }
+    u64* stage_cols = nullptr;
+    u64* stage_pairs = nullptr;
+    if (compact && !count_only) {
+        stage_cols = reinterpret_cast<u64*>(smem1 + off_b) + (size_t)warp * (2 * S1_CHUNK);
+        stage_pairs = stage_cols + S1_CHUNK;
+    }
+    BlockHists H;
+    H.cols = s_hist_cols;
+    H.pairs = s_hist_pairs;
+    H.ncols = (!count_only && p.fh_cols.hist) ? p.fh_cols.npasses : 0;
+    H.npairs = (!count_only && p.fh_pairs.hist) ? p.fh_pairs.npasses : 0;
 #pragma unroll
-    for (int q = 0; q < S1_MAX_FUSED; ++q) {
-        fsh[q] = q < nfused ? p.fh.shift[q] : 0;
-        fmk[q] = q < nfused ? (1u << p.fh.bits[q]) - 1u : 0u;
+    for (int r = 0; r < S1_MAX_FUSED; ++r) {
+        H.csh[r] = r < H.ncols ? p.fh_cols.shift[r] : 0;
+        H.cmk[r] = r < H.ncols ? (1u << p.fh_cols.bits[r]) - 1u : 0u;
     }
-    if (nfused) {
-        for (int i = tid; i < S1_MAX_FUSED * 256; i += S1_THREADS) (&s_hist[0][0])[i] = 0;
-        __syncthreads();
+#pragma unroll
+    for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
+        H.psh[r] = r < H.npairs ? p.fh_pairs.shift[r] : 0;
+        H.pmk[r] = r < H.npairs ? (1u << p.fh_pairs.bits[r]) - 1u : 0u;
     }
-    u32 n_over = 0, n_clr = 0;
+    for (int i = tid; i < S1_MAX_FUSED * 256; i += S1_THREADS) (&s_hist_cols[0][0])[i] = 0;
+    for (int i = tid; i < S1_MAX_FUSED_P * 256; i += S1_THREADS) (&s_hist_pairs[0][0])[i] = 0;
+    __syncthreads();
+
+    u32 n_over = 0, n_clr = 0, n_reg = 0;
     u64 n_kept = 0;
-    u64* const wstage = stage[warp];
+    const int kwin = n < 32 ? n : 32; // cofacet vertices n-1 .. n-kwin are tested in the row-shared window
 
     for (;;) {
         u32 chunk = 0;
@@ -73,38 +204,50 @@ __global__ void __launch_bounds__(S1_THREADS) stage1_kernel(const Stage1Params p
         decode_simplex_fast<M>(p.bt, idx, n, v); // warp-uniform
         int v0 = v[0];
         u32 wcount = 0;
+        int qcount = 0;
         bool new_upper = true;
         u32 up2 = 0xffffffffu;
 
         while (rem > 0) {
-            // ---- per row: keys among v[1..M-1], upper part of the record
+            // ---- per row: keys among v[1..M-1], upper part of the record, the shared window of U
             if (M > 2 && new_upper) {
                 up2 = 0xffffffffu;
 #pragma unroll
                 for (int a = 3; a < M; ++a)
 #pragma unroll
-                    for (int b = 2; b < a; ++b) up2 = min(up2, (u32)__ldg(Kf + v[a] * n + v[b]));
+                    for (int b = 2; b < a; ++b) up2 = min(up2, (u32)Kf[v[a] * pitch + v[b]]);
                 new_upper = false;
             }
             u32 up1 = up2;
 #pragma unroll
-            for (int a = 2; a < M; ++a) up1 = min(up1, (u32)__ldg(Kf + v[a] * n + v[1]));
+            for (int a = 2; a < M; ++a) up1 = min(up1, (u32)Kf[v[a] * pitch + v[1]]);
             u64 lowbase = 0;
 #pragma unroll
             for (int j = M - 1; j >= 1; --j) lowbase = (lowbase << vbits) | (u64)(u32)v[j];
             lowbase <<= vbits;
+            const int vtop = v[M - 1];
             const int row_len = min(v[1] - v0, rem);
+            u32 uwin = 0; // lane l: min_j>=1 key1(v_j, n-1-l)
+            if (!count_only && lane < kwin) {
+                uwin = 0xffffffffu;
+#pragma unroll
+                for (int j = 1; j < M; ++j) uwin = min(uwin, (u32)Kf[v[j] * pitch + (n - 1 - lane)]);
+            }
 
             for (int off = lane; off - lane < row_len; off += 32) {
+                if (qcount > S1_QCAP - 32) { // room for a full warp of new entries
+                    drain_queue<M, KT>(p, Kf, q, qcount, lane, stage_pairs, H, psentinel, n_reg);
+                    qcount = 0;
+                }
                 const bool valid = off < row_len;
-                const int x = v0 + off;
+                const int x = valid ? v0 + off : 0;
+                const u64 ci = idx + (u64)off;
                 bool keep = false;
                 u32 key1 = up1;
                 if (valid) {
 #pragma unroll
-                    for (int j = 1; j < M; ++j) key1 = min(key1, (u32)__ldg(Kf + v[j] * n + x));
+                    for (int j = 1; j < M; ++j) key1 = min(key1, (u32)Kf[v[j] * pitch + x]);
                     if (key1 >= thr1) {
-                        const u64 ci = idx + (u64)off;
                         bool clr;
                         if (p.clear.bitmap) clr = (__ldg(p.clear.bitmap + (ci >> 5)) >> (ci & 31)) & 1u;
                         else
@@ -116,14 +259,105 @@ __global__ void __launch_bounds__(S1_THREADS) stage1_kernel(const Stage1Params p
                         ++n_over;
                 }
                 const u32 bal = __ballot_sync(RIPS_FULL_MASK, keep);
-                if (keep && write) {
-                    const u64 rec = ((u64)(key1 - 1u) << lowbits) | lowbase | (u64)(u32)x;
-                    wstage[wcount + __popc(bal & lt_mask)] = rec;
-#pragma unroll
-                    for (int q = 0; q < S1_MAX_FUSED; ++q)
-                        if (q < nfused) atomicAdd(&s_hist[q][(u32)(rec >> fsh[q]) & fmk[q]], 1u);
-                }
+                const u32 slot = wcount + __popc(bal & lt_mask);
                 wcount += __popc(bal);
+                if (count_only) continue;
+
+                // ---- a7, fast path: cofacet vertices n-1, n-2, ... against the row's window
+                const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | lowbase | (u64)(u32)x) : csentinel;
+                int fv = -1;
+                bool open_scan = keep;
+                u32 need = bal;
+                const KT* rowx = Kf + x * pitch;
+                int k = 0;
+                while (need) {
+                    if (k >= kwin || (k >= 6 && __popc(need) <= 1)) break;
+                    const u32 uu = __shfl_sync(RIPS_FULL_MASK, uwin, k);
+                    if (open_scan) {
+                        const u32 own = (u32)rowx[n - 1 - k];
+                        if (min(uu, own) >= key1) { fv = n - 1 - k; open_scan = false; }
+                    }
+                    need = __ballot_sync(RIPS_FULL_MASK, open_scan);
+                    ++k;
+                }
+                const bool found = keep && fv >= 0;
+                const bool regular = found && fv > vtop;
+                const bool toq = keep && !found; // the scan left the window: the warp finishes it cooperatively
+                u64 prec = psentinel;
+                if (regular) {
+                    prec = ((u64)(u32)fv << p.tbits) | (ci + p.bt(fv, M + 1));
+                    ++n_reg;
+                }
+                // ---- cofacet vertex below the top of s: facet test.  The top vertex is the row's, so
+                // these lanes come in whole rows (every column of a row whose top vertex is n-1, ...)
+                bool is_irr = false, is_non = false;
+                u64 irr_rec = 0;
+                if (found && !regular) {
+                    int sv[M];
+                    sv[0] = x;
+#pragma unroll
+                    for (int j = 1; j < M; ++j) sv[j] = v[j];
+                    int fseg = 0;
+#pragma unroll
+                    for (int j = 0; j < M; ++j) fseg += (sv[j] < fv) ? 1 : 0;
+                    if (s_is_youngest_facet<M, KT>(Kf, pitch, sv, key1, fv, fseg)) {
+                        irr_rec = (cofacet_index<M>(p.bt, sv, fv, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
+                        is_irr = true;
+                    } else
+                        is_non = true;
+                }
+                const u32 b_irr = __ballot_sync(RIPS_FULL_MASK, is_irr);
+                if (b_irr) {
+                    u64 base = 0;
+                    if (lane == __ffs(b_irr) - 1)
+                        base = atomicAdd((unsigned long long*)(p.counters + S1C_IRREGULAR), (unsigned long long)__popc(b_irr));
+                    base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_irr) - 1) + __popc(b_irr & lt_mask);
+                    if (is_irr && base < p.irr_cap) p.irr_out[base] = irr_rec;
+                }
+                const u32 b_non = __ballot_sync(RIPS_FULL_MASK, is_non);
+                if (b_non) {
+                    u64 base = 0;
+                    if (lane == __ffs(b_non) - 1)
+                        base = atomicAdd((unsigned long long*)(p.counters + S1C_NONAPP), (unsigned long long)__popc(b_non));
+                    base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_non) - 1) + __popc(b_non & lt_mask);
+                    if (is_non && base < p.non_cap) p.non_out[base] = rec;
+                }
+                // ---- stores
+                if (compact) {
+                    if (keep) {
+                        stage_cols[slot] = rec;
+                        if (!toq) stage_pairs[slot] = prec;
+                    }
+                } else if (valid) {
+                    __stcs(p.cols_out + ci, rec);
+                    if (!toq) __stcs(p.pairs_out + ci, prec);
+                }
+                // ---- fused histograms over every slot written
+                const bool wrote_col = compact ? keep : valid;
+                if (wrote_col) {
+#pragma unroll
+                    for (int r = 0; r < S1_MAX_FUSED; ++r)
+                        if (r < H.ncols) atomicAdd(&H.cols[r][(u32)(rec >> H.csh[r]) & H.cmk[r]], 1u);
+                }
+                const bool wrote_pair = wrote_col && !toq;
+#pragma unroll
+                for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
+                    if (r < H.npairs) { // few distinct digits in a warp: aggregate
+                        const u32 dg = wrote_pair ? ((u32)(prec >> H.psh[r]) & H.pmk[r]) : 0xffffffffu;
+                        const u32 peers = __match_any_sync(RIPS_FULL_MASK, dg);
+                        if (wrote_pair && lane == __ffs(peers) - 1) atomicAdd(&H.pairs[r][dg], (u32)__popc(peers));
+                    }
+                }
+                // ---- queue: scans that left the window, and cofacets below the top vertex of s
+                const u32 bq = __ballot_sync(RIPS_FULL_MASK, toq);
+                if (toq) {
+                    const int qp = qcount + __popc(bq & lt_mask);
+                    q.rec[qp] = rec;
+                    q.idx[qp] = ci;
+                    q.vs[qp] = n - 1 - k;
+                    q.slot[qp] = slot;
+                }
+                qcount += __popc(bq);
             }
             idx += (u64)row_len;
             rem -= row_len;
@@ -145,37 +379,46 @@ __global__ void __launch_bounds__(S1_THREADS) stage1_kernel(const Stage1Params p
         }
 
         n_kept += wcount;
-        if (!write) continue; // count-only pass
-        // ---- ordered compaction: warp-level look-back over the chunks
-        const u64 excl = lookback_exclusive(p.status, (i64)chunk, (u64)wcount);
-        __syncwarp();
-        u64* dst = p.out + excl;
-        for (u32 i = lane; i < wcount; i += 32) __stcs(dst + i, wstage[i]);
-        __syncwarp();
+        if (count_only) continue;
+        if (qcount) drain_queue<M, KT>(p, Kf, q, qcount, lane, stage_pairs, H, psentinel, n_reg);
+        if (compact) {
+            // ---- ordered compaction: warp-level look-back over the chunks
+            const u64 excl = lookback_exclusive(p.status, (i64)chunk, (u64)wcount);
+            __syncwarp();
+            for (u32 i = lane; i < wcount; i += 32) {
+                __stcs(p.cols_out + excl + i, stage_cols[i]);
+                __stcs(p.pairs_out + excl + i, stage_pairs[i]);
+            }
+            __syncwarp();
+        }
     }
 
-    // ---- counters and the fused histogram: once per block
+    // ---- counters and the fused histograms: once per block
     n_over = warp_sum_u32(n_over);
     n_clr = warp_sum_u32(n_clr);
+    n_reg = warp_sum_u32(n_reg);
     if (lane == 0) {
-        if (n_kept) atomicAdd((unsigned long long*)&p.counters[0], (unsigned long long)n_kept);
-        if (n_over) atomicAdd((unsigned long long*)&p.counters[1], (unsigned long long)n_over);
-        if (n_clr) atomicAdd((unsigned long long*)&p.counters[2], (unsigned long long)n_clr);
+        if (n_kept) atomicAdd((unsigned long long*)&p.counters[S1C_KEPT], (unsigned long long)n_kept);
+        if (n_over) atomicAdd((unsigned long long*)&p.counters[S1C_OVER], (unsigned long long)n_over);
+        if (n_clr) atomicAdd((unsigned long long*)&p.counters[S1C_CLEARED], (unsigned long long)n_clr);
+        if (n_reg) atomicAdd((unsigned long long*)&p.counters[S1C_REGULAR], (unsigned long long)n_reg);
     }
-    if (nfused) {
-        __syncthreads();
-        for (int i = tid; i < nfused * 256; i += S1_THREADS) {
-            u32 c = (&s_hist[0][0])[i];
-            if (c) atomicAdd((unsigned long long*)&p.fh.hist[i], (unsigned long long)c);
-        }
+    __syncthreads();
+    for (int i = tid; i < H.ncols * 256; i += S1_THREADS) {
+        u32 c = (&s_hist_cols[0][0])[i];
+        if (c) atomicAdd((unsigned long long*)&p.fh_cols.hist[i], (unsigned long long)c);
+    }
+    for (int i = tid; i < H.npairs * 256; i += S1_THREADS) {
+        u32 c = (&s_hist_pairs[0][0])[i];
+        if (c) atomicAdd((unsigned long long*)&p.fh_pairs.hist[i], (unsigned long long)c);
     }
 }
 
-__global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, int shift)
+__global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, int shift, u64 mask)
 {
     i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n_rows) {
-        u64 t = __ldg(rows + i) >> shift;
+        u64 t = (__ldg(rows + i) >> shift) & mask;
         atomicOr(bitmap + (t >> 5), 1u << (t & 31));
     }
 }
@@ -183,9 +426,22 @@ __global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i
 template <int M, typename KT>
 cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 {
+    const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
+    const int k_in = (!p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
+    const size_t smem = (k_in ? kf_bytes : 0) + (size_t)S1_WARPS * S1_QCAP * 24 +
+                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * S1_CHUNK * 8 : 0);
+    auto kern = enumerate_apparent_kernel<M, KT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e != cudaSuccess) return e;
+    int per_sm = 1;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, S1_THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     i64 g = (p.tiles + S1_WARPS - 1) / S1_WARPS;
-    if (g > (i64)148 * S1_BLOCKS_PER_SM) g = (i64)148 * S1_BLOCKS_PER_SM;
-    stage1_kernel<M, KT><<<(unsigned)g, S1_THREADS, 0, st>>>(p);
+    if (g > (i64)sms * per_sm) g = (i64)sms * per_sm;
+    kern<<<(unsigned)g, S1_THREADS, smem, st>>>(p, k_in);
     return cudaGetLastError();
 }
 
@@ -206,10 +462,10 @@ cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t
 #undef S1_CASE
 }
 
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, cudaStream_t st)
+cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st)
 {
     if (n_rows == 0) return cudaSuccess;
     i64 blocks = (n_rows + 255) / 256;
-    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, rows, n_rows, shift);
+    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, rows, n_rows, shift, mask);
     return cudaGetLastError();
 }

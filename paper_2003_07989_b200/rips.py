@@ -29,7 +29,7 @@ SYMBOLS = [
 class RipsStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in (
         "n_candidates", "n_removed_by_diameter", "n_cleared", "n_columns", "n_apparent", "n_nonapparent",
-        "n_reduced_pivots", "n_essential", "n_additions", "n_bars")] + [(k, C.c_int32) for k in (
+        "n_reduced_pivots", "n_essential", "n_additions", "n_bars", "n_slots", "n_regular")] + [(k, C.c_int32) for k in (
         "key_bits", "index_bits", "sort_passes", "pair_sort_passes")]
 
     def as_dict(self):
