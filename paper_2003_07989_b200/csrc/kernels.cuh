@@ -65,6 +65,7 @@ struct Stage1Params {
     int n;
     u64 total;        // C(n, d+1)
     i64 tiles;        // warp chunks
+    int chunk;        // candidates per warp chunk (stage1_chunk)
     u32 thr_key;      // keep iff key >= thr_key
     u32 sentinel_key; // key field of the column sentinel (= number of distinct keys, larger than every key)
     int vbits, lowbits;
@@ -73,6 +74,7 @@ struct Stage1Params {
     int compact;      // 0: one slot per candidate, sentinels in the dropped ones (sorted away afterwards);
                       // 1: survivors compacted in increasing index with a decoupled look-back
     int count_only;   // 1: only counters[S1C_KEPT/OVER/CLEARED] are produced
+    int fast_visits;  // cofacet vertices each lane tests on its own before the warp takes over its scan (<= 32)
     u64* cols_out;    // packed column records
     u64* pairs_out;   // same slots: regular pair record (v << tbits) | cidx(t), or the pair sentinel (n << tbits)
     u64* irr_out;     // irregular apparent pairs (cidx(t) << 3) | j, unordered; capacity irr_cap
@@ -84,7 +86,7 @@ struct Stage1Params {
     FusedHist fh_cols;   // digit histogram of the filtration sort (over every slot written to cols_out)
     FusedHist fh_pairs;  // digit histogram of the partition of pairs_out by v
 };
-i64 stage1_tiles(u64 total);
+int stage1_chunk(u64 total);
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
 // bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask
 cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st);

@@ -5,12 +5,14 @@
 // in increasing combinatorial index leave each pass in increasing index within equal digits: the
 // index bits never have to be sorted.
 #include "radix_sort.cuh"
+#include <cstdlib>
 
 namespace {
 
 constexpr int SORT_THREADS = 512;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
 constexpr int SORT_IPT = 12;
 constexpr int SORT_MIN_BLOCKS = 2;
+constexpr int SORT_LB_BATCH = 8;     // predecessor tiles read per look-back step
 constexpr int SORT_RANK_BATCH = 6;   // records ranked per pipelined batch (divides SORT_IPT)
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
@@ -90,6 +92,7 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 // look-back at once, scan over the bins; (4) records placed in tile-sorted order in shared memory;
 // (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
+template <bool MATCH>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
                      const u64* __restrict__ global_base, u64* status, u32* ticket)
@@ -137,8 +140,26 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
 #pragma unroll
     for (int h = 0; h < SORT_IPT; h += SORT_RANK_BATCH) {
 #pragma unroll
-        for (int i = h; i < h + SORT_RANK_BATCH; ++i)
-            rank[i] = __match_any_sync(RIPS_FULL_MASK, (u32)(key[i] >> shift) & mask);
+        for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
+            const u32 d = (u32)(key[i] >> shift) & mask;
+            if (MATCH) {
+                // one MATCH per record: ~2 cycles per DISTINCT digit in the warp (measured), so only for
+                // skewed digits (the partition of the pairs by cofacet vertex)
+                rank[i] = __match_any_sync(RIPS_FULL_MASK, d);
+            } else {
+                // one ballot per digit bit: flat cost, cheaper than MATCH once a warp holds many digits
+                u32 peers = RIPS_FULL_MASK;
+#pragma unroll
+                for (int b = 0; b < 8; ++b) {
+                    if (b < bits) {
+                        const bool bit = (d >> b) & 1u;
+                        const u32 bal = __ballot_sync(RIPS_FULL_MASK, bit);
+                        peers &= bit ? bal : ~bal;
+                    }
+                }
+                rank[i] = peers;
+            }
+        }
         u32 old[SORT_RANK_BATCH];
 #pragma unroll
         for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
@@ -193,18 +214,30 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
         stage[bin_start[d] + wh[d] + rank[i]] = key[i];
     }
 
-    // ---- (5) decoupled look-back, one thread per bin
+    // ---- (5) decoupled look-back, one thread per bin.  The tiles in flight finish their ranking at
+    // about the same time, so the nearest inclusive prefix is usually many tiles back; LB_BATCH
+    // predecessors are read at once (independent loads) so that the walk costs one L2 round trip per
+    // batch instead of one per tile.
     if (tid < nbins) {
         u64 excl = 0;
         if (tile > 0) {
             i64 t = tile - 1;
-            for (;;) {
-                u64 s = ld_volatile_u64(status + t * nbins + tid);
-                u64 flag = s >> 62;
-                if (flag == 0) continue;
-                excl += s & LB_VALUE_MASK;
-                if (flag == 2) break;
-                --t;
+            bool done = false;
+            while (!done) {
+                u64 sv[SORT_LB_BATCH];
+#pragma unroll
+                for (int b = 0; b < SORT_LB_BATCH; ++b)
+                    sv[b] = (t - b >= 0) ? ld_volatile_u64(status + (t - b) * nbins + tid) : LB_FLAG_INC;
+#pragma unroll
+                for (int b = 0; b < SORT_LB_BATCH; ++b) {
+                    if (!done) {
+                        const u64 flag = sv[b] >> 62;
+                        if (flag == 0) break; // not published yet: poll again from this tile
+                        excl += sv[b] & LB_VALUE_MASK;
+                        --t;
+                        if (flag == 2) done = true;
+                    }
+                }
             }
             st_volatile_u64(status + tile * nbins + tid, LB_FLAG_INC | (excl + (u64)my_count));
         }
@@ -283,7 +316,7 @@ cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream)
 }
 
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream, u64** result,
-                     SortTimes* times, i64* launches, bool hist_ready)
+                     SortTimes* times, i64* launches, bool hist_ready, bool skewed_digits)
 {
     *result = a;
     if (times && times->enabled) cudaEventRecord(times->ev[0], stream);
@@ -293,14 +326,19 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     }
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)pass_smem_bytes(8));
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(onesweep_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)pass_smem_bytes(8));
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(sort_histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 4);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
+    static const int force_rank = getenv("RIPS_SORT_RANK") ? atoi(getenv("RIPS_SORT_RANK")) : 1; // tuning: 0 ballots, 1 match
+    if (force_rank >= 0) skewed_digits = force_rank != 0;
     ScratchLayout L = scratch_layout(n, plan);
     unsigned char* sc = (unsigned char*)scratch;
     u64* hist = (u64*)(sc + L.hist_off);
@@ -332,8 +370,12 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         size_t status_bytes = (size_t)tiles * ((size_t)1 << plan.bits[p]) * 8;
         e = cudaMemsetAsync(status, 0, status_bytes, stream);
         if (e != cudaSuccess) return e;
-        onesweep_pass_kernel<<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-            src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p);
+        if (skewed_digits)
+            onesweep_pass_kernel<true><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
+                src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p);
+        else
+            onesweep_pass_kernel<false><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
+                src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p);
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }

@@ -31,7 +31,9 @@ struct SortTimes {
 // hist_ready: the caller zeroed the scratch head with sort_prepare_fused and a producer kernel has
 // already accumulated the raw digit counts of every pass into sort_hist_ptr(scratch)[pass][256]
 // (FusedHist in kernels.cuh); the sort then skips its own histogram read of the records.
+// skewed_digits: a warp's 32 records mostly share a few digits (ranking by MATCH instead of ballots).
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
-                     u64** result, SortTimes* times, i64* launches, bool hist_ready = false);
+                     u64** result, SortTimes* times, i64* launches, bool hist_ready = false,
+                     bool skewed_digits = false);
 cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream);
 u64* sort_hist_ptr(void* scratch);

@@ -101,6 +101,7 @@ struct rips_ctx {
     u32* d_K = nullptr;
     void* d_Kf = nullptr;  // full symmetric matrix of key+1 (common.cuh)
     int kf_u16 = 0, kf_pitch = 1, vbits = 1;
+    int fast_visits = 0; // tuning override (RIPS_FAST_VISITS), 0 = per-dimension default
     float* d_values = nullptr;
     u64* d_binom = nullptr;
     u64* d_counters = nullptr; // 8 u64 scratch counters
@@ -343,7 +344,8 @@ int run_stage1(rips_ctx* c, int d)
     // q of admissible edges (q^(edges of the simplex)) and compact when most are dropped
     const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
     s.compact = (c->thr_key != 0 && std::pow(q, (double)(s.M * (s.M - 1) / 2)) < 0.5) ? 1 : 0;
-    const i64 tiles = stage1_tiles(s.total);
+    const int chunk = stage1_chunk(s.total);
+    const i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
     Stage1Params p;
     p.Kf = c->d_Kf;
     p.pitch = c->kf_pitch;
@@ -351,6 +353,7 @@ int run_stage1(rips_ctx* c, int d)
     p.n = (int)n;
     p.total = s.total;
     p.tiles = tiles;
+    p.chunk = chunk;
     p.thr_key = c->thr_key;
     p.sentinel_key = c->n_distinct;
     p.vbits = c->vbits;
@@ -359,6 +362,7 @@ int run_stage1(rips_ctx* c, int d)
     p.clear = cs;
     p.compact = s.compact;
     p.count_only = 0;
+    p.fast_visits = c->fast_visits > 0 ? c->fast_visits : (s.M >= 4 ? 8 : s.M == 3 ? 12 : 16);
     p.cols_out = p.pairs_out = p.irr_out = p.non_out = nullptr;
     p.irr_cap = p.non_cap = 0;
     p.status = nullptr;
@@ -396,8 +400,10 @@ int run_stage1(rips_ctx* c, int d)
     RC(ensure(c, s.pair_scratch, sort_scratch_bytes((i64)cap, s.pair_plan)));
     const bool fused = plan.npasses <= 3;           // S1_MAX_FUSED digits
     s.pair_fused = s.pair_plan.npasses <= 2;        // S1_MAX_FUSED_P digits
-    u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 64));
-    u64 non_cap = std::max<u64>(s.nonA.cap / 8, std::max<u64>(4096, cap / 16));
+    // provisioned for (d+1)/n of the columns to hold the top vertices (those pairs are irregular) and as many
+    // non-apparent ones; a run that needs more is repeated once with the exact sizes
+    u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 8));
+    u64 non_cap = std::max<u64>(s.nonA.cap / 8, std::max<u64>(4096, cap / 8));
     for (int attempt = 0;; ++attempt) {
         RC(ensure(c, s.irrA, (size_t)irr_cap * 8));
         RC(ensure(c, s.nonA, (size_t)non_cap * 8));
@@ -502,7 +508,7 @@ int run_stage2(rips_ctx* c, int d)
     s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
     u64* res = nullptr;
     CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, c->stream, &res, &st,
-                &c->launches, s.pair_fused));
+                &c->launches, s.pair_fused, true));
     s.reg = res;
     ev_record(c, s, EV_S2_END);
     s.pairs_fresh = false;
@@ -753,6 +759,7 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     c->threshold = threshold;
     c->stream = (cudaStream_t)stream;
     c->kmax = dim_max + 3;
+    if (const char* e = getenv("RIPS_FAST_VISITS")) c->fast_visits = atoi(e);
     build_binom(n, c->kmax, c->h_binom);
     if (hbinom(c, n, dim_max + 2) >> 62) { delete c; return RIPS_EOVERFLOW; }
     c->dims.resize((size_t)dim_max + 2);

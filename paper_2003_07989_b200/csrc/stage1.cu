@@ -28,11 +28,10 @@ namespace {
 
 constexpr int S1_THREADS = 512;
 constexpr int S1_WARPS = S1_THREADS / 32;
-constexpr int S1_CHUNK = 512;          // candidates per warp chunk = unit of the look-back chain
-constexpr int S1_QCAP = 64;            // queue entries per warp (drained when fewer than 32 are free)
+constexpr int S1_CHUNK = 512;          // most candidates per warp chunk (unit of work and of the look-back chain)
 constexpr int S1_MAX_FUSED = 3;        // digits of the filtration sort histogrammed on the way out
 constexpr int S1_MAX_FUSED_P = 2;      // digits of the pair partition
-constexpr size_t S1_KF_SMEM_LIMIT = 80 * 1024;   // two blocks per SM with the queues beside it
+constexpr size_t S1_KF_SMEM_LIMIT = 100 * 1024;  // two blocks per SM
 
 __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int shift, u64 x)
 {
@@ -44,13 +43,6 @@ __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int 
     }
     return lo < n && (__ldg(a + lo) >> shift) == x;
 }
-
-struct WarpQueue {
-    u64* rec;   // column record
-    u64* idx;   // cidx(s)
-    int* vs;    // first cofacet vertex still to test
-    u32* slot;  // compact mode: slot in the warp's staging arrays
-};
 
 // append `val` to a global list with capacity `cap`; the counter keeps counting past the capacity
 __device__ __forceinline__ void list_append(u64* list, u64 cap, u64* counter, u64 val)
@@ -71,69 +63,13 @@ struct BlockHists {
     u32 pmk[S1_MAX_FUSED_P];
 };
 
-// Warp-cooperative drain of the queue: per entry, 32 cofacet vertices are tested per step (lane l
-// takes v = base - l, so the reads of Kf are consecutive), then the warp-uniform classification:
-// regular pair, irregular pair (facet test), or non-apparent column.
-template <int M, typename KT>
-__device__ __forceinline__ void drain_queue(const Stage1Params& p, const KT* Kf, const WarpQueue& q, int qcount, int lane,
-                                            u64* stage_pairs, const BlockHists& H, u64 psentinel, u32& n_reg)
-{
-    __syncwarp();
-    for (int e = 0; e < qcount; ++e) {
-        const u64 rec = q.rec[e];
-        const u64 idx = q.idx[e];
-        const int vs = q.vs[e];
-        const u32 key1 = (u32)(rec >> p.lowbits) + 1u;
-        int s[M];
-        unpack_vertices<M>(rec, p.vbits, s);
-        int fv = -1;
-        for (int base = vs; base >= 0; base -= 32) {
-            const int vv = base - lane;
-            bool ok = false;
-            if (vv >= 0) {
-                u32 m = 0xffffffffu;
-#pragma unroll
-                for (int j = 0; j < M; ++j) m = min(m, (u32)Kf[s[j] * p.pitch + vv]);
-                ok = m >= key1;
-            }
-            const u32 b = __ballot_sync(RIPS_FULL_MASK, ok);
-            if (b) { fv = base - (__ffs(b) - 1); break; }
-        }
-        u64 prec = psentinel;
-        bool is_non = true;
-        u64 irr = 0;
-        if (fv >= 0) {
-            int fseg = 0;
-#pragma unroll
-            for (int j = 0; j < M; ++j) fseg += (s[j] < fv) ? 1 : 0;
-            if (fseg == M) {
-                prec = ((u64)(u32)fv << p.tbits) | (idx + p.bt(fv, M + 1));
-                is_non = false;
-                if (lane == 0) ++n_reg;
-            } else if (s_is_youngest_facet<M, KT>(Kf, p.pitch, s, key1, fv, fseg)) {
-                irr = (cofacet_index<M>(p.bt, s, fv, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
-                is_non = false;
-                if (lane == 0) list_append(p.irr_out, p.irr_cap, p.counters + S1C_IRREGULAR, irr);
-            }
-        }
-        if (lane == 0) {
-            if (is_non) list_append(p.non_out, p.non_cap, p.counters + S1C_NONAPP, rec);
-            if (p.compact) stage_pairs[q.slot[e]] = prec;
-            else __stcs(p.pairs_out + idx, prec);
-#pragma unroll
-            for (int r = 0; r < S1_MAX_FUSED_P; ++r)
-                if (r < H.npairs) atomicAdd(&H.pairs[r][(u32)(prec >> H.psh[r]) & H.pmk[r]], 1u);
-        }
-    }
-    __syncwarp();
-}
-
 template <int M, typename KT>
 __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const Stage1Params p, int k_in_smem)
 {
     extern __shared__ __align__(16) unsigned char smem1[];
     __shared__ u32 s_hist_cols[S1_MAX_FUSED][256];
     __shared__ u32 s_hist_pairs[S1_MAX_FUSED_P][256];
+    __shared__ u32 s_uwin[S1_WARPS][32];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = p.n, pitch = p.pitch, vbits = p.vbits, lowbits = p.lowbits;
@@ -143,7 +79,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     const u64 csentinel = (u64)p.sentinel_key << lowbits;
     const u64 psentinel = (u64)(u32)n << p.tbits;
 
-    // ---- shared memory carve-up: [Kf] [queues] [staging (compact mode)]
+    // ---- shared memory carve-up: [Kf] [staging (compact mode)]
     size_t off_b = 0;
     const KT* Kf = reinterpret_cast<const KT*>(p.Kf);
     if (k_in_smem) {
@@ -153,15 +89,6 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
         for (int i = tid; i < cnt16; i += S1_THREADS) dst[i] = __ldg(src + i);
         Kf = reinterpret_cast<const KT*>(smem1);
         off_b = (size_t)cnt16 * 16;
-    }
-    WarpQueue q;
-    {
-        unsigned char* qb = smem1 + off_b + (size_t)warp * (S1_QCAP * 24);
-        q.rec = reinterpret_cast<u64*>(qb);
-        q.idx = q.rec + S1_QCAP;
-        q.vs = reinterpret_cast<int*>(q.idx + S1_QCAP);
-        q.slot = reinterpret_cast<u32*>(q.vs + S1_QCAP);
-        off_b += (size_t)S1_WARPS * (S1_QCAP * 24);
     }
     u64* stage_cols = nullptr;
     u64* stage_pairs = nullptr;
@@ -190,7 +117,9 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
 
     u32 n_over = 0, n_clr = 0, n_reg = 0;
     u64 n_kept = 0;
-    const int kwin = n < 32 ? n : 32; // cofacet vertices n-1 .. n-kwin are tested in the row-shared window
+    const int kwin = n < 32 ? n : 32;
+    const int kfast = p.fast_visits < kwin ? p.fast_visits : kwin; // vertices n-1 .. n-kfast: per-lane scan of the row's window
+    u32* const uw = s_uwin[warp];
 
     for (;;) {
         u32 chunk = 0;
@@ -198,13 +127,12 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
         chunk = __shfl_sync(RIPS_FULL_MASK, chunk, 0);
         if ((i64)chunk >= p.tiles) break;
 
-        u64 idx = (u64)chunk * S1_CHUNK;
-        int rem = (p.total - idx) < (u64)S1_CHUNK ? (int)(p.total - idx) : S1_CHUNK;
+        u64 idx = (u64)chunk * (u64)p.chunk;
+        int rem = (p.total - idx) < (u64)p.chunk ? (int)(p.total - idx) : p.chunk;
         int v[M];
         decode_simplex_fast<M>(p.bt, idx, n, v); // warp-uniform
         int v0 = v[0];
         u32 wcount = 0;
-        int qcount = 0;
         bool new_upper = true;
         u32 up2 = 0xffffffffu;
 
@@ -227,18 +155,21 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
             lowbase <<= vbits;
             const int vtop = v[M - 1];
             const int row_len = min(v[1] - v0, rem);
-            u32 uwin = 0; // lane l: min_j>=1 key1(v_j, n-1-l)
-            if (!count_only && lane < kwin) {
-                uwin = 0xffffffffu;
+            // window of the row: uw[l] = min_j>=1 key1(v_j, n-1-l), the part of the cofacet test of vertex
+            // n-1-l that every column of the row shares
+            if (!count_only) {
+                __syncwarp();
+                u32 u = 0;
+                if (lane < kwin) {
+                    u = 0xffffffffu;
 #pragma unroll
-                for (int j = 1; j < M; ++j) uwin = min(uwin, (u32)Kf[v[j] * pitch + (n - 1 - lane)]);
+                    for (int j = 1; j < M; ++j) u = min(u, (u32)Kf[v[j] * pitch + (n - 1 - lane)]);
+                }
+                uw[lane] = u;
+                __syncwarp();
             }
 
             for (int off = lane; off - lane < row_len; off += 32) {
-                if (qcount > S1_QCAP - 32) { // room for a full warp of new entries
-                    drain_queue<M, KT>(p, Kf, q, qcount, lane, stage_pairs, H, psentinel, n_reg);
-                    qcount = 0;
-                }
                 const bool valid = off < row_len;
                 const int x = valid ? v0 + off : 0;
                 const u64 ci = idx + (u64)off;
@@ -266,23 +197,37 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 // ---- a7, fast path: cofacet vertices n-1, n-2, ... against the row's window
                 const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | lowbase | (u64)(u32)x) : csentinel;
                 int fv = -1;
-                bool open_scan = keep;
-                u32 need = bal;
                 const KT* rowx = Kf + x * pitch;
-                int k = 0;
-                while (need) {
-                    if (k >= kwin || (k >= 6 && __popc(need) <= 1)) break;
-                    const u32 uu = __shfl_sync(RIPS_FULL_MASK, uwin, k);
-                    if (open_scan) {
-                        const u32 own = (u32)rowx[n - 1 - k];
-                        if (min(uu, own) >= key1) { fv = n - 1 - k; open_scan = false; }
+                if (keep) { // each lane on its own, up to kfast vertices (the common case ends after one or two)
+                    for (int k = 0; k < kfast; ++k) {
+                        if (min(uw[k], (u32)rowx[n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
                     }
-                    need = __ballot_sync(RIPS_FULL_MASK, open_scan);
-                    ++k;
+                }
+                // the lanes still scanning are finished by the whole warp, one after the other: 32 cofacet
+                // vertices per step (lane l takes vertex base - l, so all reads of Kf are consecutive)
+                u32 open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
+                while (open) {
+                    const int src = __ffs(open) - 1;
+                    open &= open - 1;
+                    const int xs = __shfl_sync(RIPS_FULL_MASK, x, src);
+                    const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
+                    int res = -1;
+                    for (int base = n - 1 - kfast; base >= 0; base -= 32) {
+                        const int vv = base - lane;
+                        bool ok = false;
+                        if (vv >= 0) {
+                            u32 m = (u32)Kf[xs * pitch + vv];
+#pragma unroll
+                            for (int j = 1; j < M; ++j) m = min(m, (u32)Kf[v[j] * pitch + vv]);
+                            ok = m >= ks;
+                        }
+                        const u32 b = __ballot_sync(RIPS_FULL_MASK, ok);
+                        if (b) { res = base - (__ffs(b) - 1); break; }
+                    }
+                    if (lane == src) fv = res;
                 }
                 const bool found = keep && fv >= 0;
                 const bool regular = found && fv > vtop;
-                const bool toq = keep && !found; // the scan left the window: the warp finishes it cooperatively
                 u64 prec = psentinel;
                 if (regular) {
                     prec = ((u64)(u32)fv << p.tbits) | (ci + p.bt(fv, M + 1));
@@ -290,7 +235,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 }
                 // ---- cofacet vertex below the top of s: facet test.  The top vertex is the row's, so
                 // these lanes come in whole rows (every column of a row whose top vertex is n-1, ...)
-                bool is_irr = false, is_non = false;
+                bool is_irr = false, is_non = keep && !found;
                 u64 irr_rec = 0;
                 if (found && !regular) {
                     int sv[M];
@@ -326,11 +271,11 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 if (compact) {
                     if (keep) {
                         stage_cols[slot] = rec;
-                        if (!toq) stage_pairs[slot] = prec;
+                        stage_pairs[slot] = prec;
                     }
                 } else if (valid) {
                     __stcs(p.cols_out + ci, rec);
-                    if (!toq) __stcs(p.pairs_out + ci, prec);
+                    __stcs(p.pairs_out + ci, prec);
                 }
                 // ---- fused histograms over every slot written
                 const bool wrote_col = compact ? keep : valid;
@@ -339,7 +284,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                     for (int r = 0; r < S1_MAX_FUSED; ++r)
                         if (r < H.ncols) atomicAdd(&H.cols[r][(u32)(rec >> H.csh[r]) & H.cmk[r]], 1u);
                 }
-                const bool wrote_pair = wrote_col && !toq;
+                const bool wrote_pair = wrote_col;
 #pragma unroll
                 for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
                     if (r < H.npairs) { // few distinct digits in a warp: aggregate
@@ -348,16 +293,6 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                         if (wrote_pair && lane == __ffs(peers) - 1) atomicAdd(&H.pairs[r][dg], (u32)__popc(peers));
                     }
                 }
-                // ---- queue: scans that left the window, and cofacets below the top vertex of s
-                const u32 bq = __ballot_sync(RIPS_FULL_MASK, toq);
-                if (toq) {
-                    const int qp = qcount + __popc(bq & lt_mask);
-                    q.rec[qp] = rec;
-                    q.idx[qp] = ci;
-                    q.vs[qp] = n - 1 - k;
-                    q.slot[qp] = slot;
-                }
-                qcount += __popc(bq);
             }
             idx += (u64)row_len;
             rem -= row_len;
@@ -380,7 +315,6 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
 
         n_kept += wcount;
         if (count_only) continue;
-        if (qcount) drain_queue<M, KT>(p, Kf, q, qcount, lane, stage_pairs, H, psentinel, n_reg);
         if (compact) {
             // ---- ordered compaction: warp-level look-back over the chunks
             const u64 excl = lookback_exclusive(p.status, (i64)chunk, (u64)wcount);
@@ -428,7 +362,7 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 {
     const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
     const int k_in = (!p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
-    const size_t smem = (k_in ? kf_bytes : 0) + (size_t)S1_WARPS * S1_QCAP * 24 +
+    const size_t smem = (k_in ? kf_bytes : 0) +
                         ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * S1_CHUNK * 8 : 0);
     auto kern = enumerate_apparent_kernel<M, KT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -447,7 +381,15 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 
 } // namespace
 
-i64 stage1_tiles(u64 total) { return (i64)((total + S1_CHUNK - 1) / S1_CHUNK); } // warp chunks
+// Candidates per warp chunk: S1_CHUNK when there is plenty of work, less (a multiple of 32) when the
+// index space is small, so that every SM still gets warps to run.
+int stage1_chunk(u64 total)
+{
+    u64 c = (total / (148ull * 64) + 31) / 32 * 32;
+    if (c < 32) c = 32;
+    if (c > (u64)S1_CHUNK) c = S1_CHUNK;
+    return (int)c;
+}
 
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st)
 {
