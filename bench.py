@@ -189,6 +189,47 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+# ------------------------------------------------------------------------------------ ranks
+class Ranks:
+    """One process per GPU (replicas only): rendezvous, barrier and the max over
+    ranks of a device time.  backend "nccl" on the GPU box, "gloo" in the CPU test."""
+
+    def __init__(self, backend="nccl", device=None):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist = torch, dist
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.device = device
+        if self.world > 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29533")
+            kw = {"device_id": device} if (backend == "nccl" and device is not None) else {}
+            dist.init_process_group(backend, rank=self.rank, world_size=self.world, **kw)
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        if self.device is not None and self.device.type == "cuda":
+            self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, x):
+        if self.world == 1:
+            return float(x)
+        t = self.torch.tensor([float(x)], dtype=self.torch.float64, device=self.device or "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def whole_job_rate(self, units_per_rank, ms):
+        """units all ranks processed / the slowest rank's time"""
+        return self.world * units_per_rank / (self.max_over_ranks(ms) * 1e-3)
+
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------ B200 arm
 KERNELS = {  # rips_timings field -> kernel
     "enumerate_ms": "enumerate_apparent_kernel (a3-a5+a7 fused enumerate, filter, apparent test)",
@@ -210,23 +251,14 @@ def algorithmic_bytes(field, st):
 
 def run_b200(args):
     import torch
-    import torch.distributed as dist
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product has no CPU fallback"
     torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ranks = Ranks("nccl", torch.device("cuda", local))
+    rank, world, barrier = ranks.rank, ranks.world, ranks.barrier
     from paper_2003_07989_b200 import inputs, rips
     rips.lib()
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
 
     w = inputs.config(args.config)
     D = w.dim_max
@@ -276,11 +308,7 @@ def run_b200(args):
     elapsed_ms = ev0.elapsed_time(ev1)
     launches = g.kernel_launches() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        tt = torch.tensor([elapsed_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tt.item())
-    ms_per_step = elapsed_ms / args.steps
+    ms_per_step = ranks.max_over_ranks(elapsed_ms) / args.steps
     value = world * n_cand / (ms_per_step * 1e-3)
 
     # ---- roofline of the dominant kernel (largest share of the timed region)
@@ -328,10 +356,7 @@ def run_b200(args):
                  "bars": {str(d): int(b.shape[0]) for d, b in enumerate(bars)}}
         h.free()
     e2e_t = statistics.median(e2e_ms) if e2e_ms else float("nan")
-    if world > 1:
-        tt = torch.tensor([e2e_t], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_t = float(tt.item())
+    e2e_t = ranks.max_over_ranks(e2e_t)
     e2e = {"value": world * n_cand / (e2e_t * 1e-3), "unit": UNIT, "ms": e2e_t,
            "h2d_bytes_per_step": int(host.numel() * 4), "d2h_bytes_per_step": int(d2h_bytes),
            "what": "rips_init(host matrix) + rips_compute + rips_barcodes(host) + rips_free"}
@@ -356,8 +381,7 @@ def run_b200(args):
                 "device_bytes": g.device_bytes(), "parallelism": "replicas" if world > 1 else "single"}
         print(json.dumps(line))
     g.free()
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
     return 0
 
 

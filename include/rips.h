@@ -119,6 +119,12 @@ int rips_stage2(rips_ctx* ctx, int d);
 /* Reduction of the non-apparent columns of dimension d (after rips_stage2(d)); completes the pivots
  * of dimension d.  Not the hot path: runs Algorithm 2 serially on the host, timed separately. */
 int rips_reduce(rips_ctx* ctx, int d);
+/* Alternative to rips_reduce(d) for a reduction done elsewhere (the paper's own split runs it on the
+ * host): installs `count` pivots (t_host[i], s_host[i]), HOST arrays ascending by t, as the
+ * pivots of dimension d that are not apparent pairs (the third layer of the pair store).  They join the
+ * apparent pairs in rips_pivots / rips_pivot_lookup and in the clearing set of dimension d+1.  No bars
+ * are produced for dimension d.  Needs rips_stage2(d).  RIPS_EINVAL if t is not strictly ascending. */
+int rips_import_pivots(rips_ctx* ctx, int d, const uint64_t* t_host, const uint64_t* s_host, int64_t count);
 
 /* Bars of dimension d: 2*count floats (birth, death) on the HOST; death = +INFINITY for essential
  * classes; zero-length bars omitted.  Order: d = 0: by ascending index of the merging edge, then

@@ -18,8 +18,12 @@
  *                  PAPER.md:443-469, increasing cidx), stop at the first with diam == diam(s);
  *                  apparent iff that facet is s (reading R3).
  *   oracle_dim0    H_0 by union-find over edges in filtration order.
- *   oracle_reduce  Implicit cohomology reduction of coboundary columns, Algorithm 2
- *                   over Z/2, columns = cofacets with diam <= threshold.
+ *   oracle_reduce  Implicit cohomology reduction of coboundary columns over Z/2, columns = cofacets
+ *                  with diam <= threshold: the standard reduction R_j <- R_j + R_i of Algorithm 1
+ *                  (PAPER.md:99-121), which Lemma 3 proves equivalent to the oblivious
+ *                  Algorithm 2; the reduced columns are kept because the oblivious
+ *                  form, which re-adds D_i, needs orders of magnitude more additions on "difficult"
+ *                  inputs such as config 3's random matrices.
  *
  * No blocking, fusion or reordering beyond what those passages state.  The only concession to
  * run time is `#pragma omp parallel for` over independent simplices (Corollary 8)
@@ -490,35 +494,56 @@ int oracle_reduce(const float *D, int n, int d, float threshold, const u64 *col_
 {
     binom_t b;
     binom_init(&b, n, d + 2);
-    map_t map = {0, 0, 0, 0};
+    map_t map = {0, 0, 0, 0};      /* cidx(t) -> position j of the column that owns the pivot */
     heap_t h = {0, 0, 0};
     u64 *pt = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
     u64 *ps = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
     u64 *es = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
+    /* R_j of the columns reduced here, kept as Algorithm 1 keeps them: the entries of
+     * the working column when its pivot was found, equal entries cancelled in pairs. */
+    col_t **Rcol = (col_t **)calloc((size_t)(ncols ? ncols : 1), sizeof(col_t *));
+    size_t *Rlen = (size_t *)calloc((size_t)(ncols ? ncols : 1), sizeof(size_t));
     i64 np = 0, ne = 0, adds = 0;
     for (i64 j = 0; j < ncols; ++j) {
         h.n = 0;
-        push_coboundary(&h, D, &b, n, d, col_cidx[j], threshold);     /* R[j] <- D_j */
+        push_coboundary(&h, D, &b, n, d, col_cidx[j], threshold);     /* R_j <- D_j */
         for (;;) {
             col_t piv;
             if (!heap_pop_pivot(&h, &piv)) { es[ne++] = col_cidx[j]; break; }   /* zero column */
-            u64 s2;
-            int found = map_get(&map, piv.cidx, &s2);
-            if (!found && n_known) {
+            u64 owner;
+            if (map_get(&map, piv.cidx, &owner)) {                    /* R_j <- R_j + R_i, i = lookup[low(R_j)] */
+                heap_push(&h, piv);
+                for (size_t e = 0; e < Rlen[owner]; ++e) heap_push(&h, Rcol[owner][e]);
+                ++adds;
+                continue;
+            }
+            int found = 0;
+            u64 s2 = 0;
+            if (n_known) {
                 i64 lo = 0, hi = n_known;
                 while (lo < hi) { i64 mid = lo + (hi - lo) / 2; if (known_t[mid] < piv.cidx) lo = mid + 1; else hi = mid; }
                 if (lo < n_known && known_t[lo] == piv.cidx) { found = 1; s2 = known_s[lo]; }
             }
-            if (!found) {                                             /* lookup[low(R[j])] <- j */
-                map_put(&map, piv.cidx, col_cidx[j]);
-                pt[np] = piv.cidx; ps[np] = col_cidx[j]; ++np;
-                break;
+            if (found) {              /* an apparent column needs no additions: R_i = D_i */
+                heap_push(&h, piv);
+                push_coboundary(&h, D, &b, n, d, s2, threshold);
+                ++adds;
+                continue;
             }
-            heap_push(&h, piv);                                       /* R[j] <- R[j] + D_lookup[low] */
-            push_coboundary(&h, D, &b, n, d, s2, threshold);
-            ++adds;
+            map_put(&map, piv.cidx, (u64)j);                          /* lookup[low(R_j)] <- j */
+            pt[np] = piv.cidx; ps[np] = col_cidx[j]; ++np;
+            Rcol[j] = (col_t *)malloc(sizeof(col_t) * (h.n + 1));
+            Rcol[j][0] = piv;
+            Rlen[j] = 1;
+            {   /* the rest of the column, equal entries cancelled in pairs */
+                col_t e;
+                while (heap_pop_pivot(&h, &e)) Rcol[j][Rlen[j]++] = e;
+            }
+            break;
         }
     }
+    for (i64 j = 0; j < ncols; ++j) free(Rcol[j]);
+    free(Rcol); free(Rlen);
     free(h.a); free(map.k); free(map.v);
     binom_free(&b);
     *piv_t = pt; *piv_s = ps; *n_piv = np; *ess_s = es; *n_ess = ne;

@@ -802,6 +802,33 @@ int rips_stage1(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_stage1(
 int rips_stage2(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_stage2(c, d); }
 int rips_reduce(rips_ctx* c, int d) { RC(check_dim(c, d, 1)); return run_reduce(c, d); }
 
+int rips_import_pivots(rips_ctx* c, int d, const uint64_t* t_host, const uint64_t* s_host, int64_t count)
+{
+    RC(check_dim(c, d, 1));
+    if (count < 0 || (count > 0 && (!t_host || !s_host))) return RIPS_EINVAL;
+    DimState& s = c->dims[d];
+    if (!s.have_s2) { g_last_error = "rips_import_pivots: rips_stage2 has not run for this dimension"; return RIPS_EINVAL; }
+    for (int64_t i = 1; i < count; ++i)
+        if (t_host[i] <= t_host[i - 1]) return RIPS_EINVAL;
+    s.have_red = false;
+    invalidate_views(s, false, false, false, true);
+    RC(ensure(c, s.red_t, (size_t)count * 8));
+    RC(ensure(c, s.red_s, (size_t)count * 8));
+    if (count) {
+        CU(cudaMemcpyAsync(s.red_t.p, t_host, (size_t)count * 8, cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(s.red_s.p, s_host, (size_t)count * 8, cudaMemcpyHostToDevice, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    s.n_red = count;
+    s.bars.clear();
+    s.stats.n_reduced_pivots = count;
+    s.stats.n_essential = 0;
+    s.stats.n_additions = 0;
+    s.stats.n_bars = 0;
+    s.have_red = true;
+    return RIPS_OK;
+}
+
 int rips_compute(rips_ctx* c)
 {
     if (!c) return RIPS_EINVAL;

@@ -19,7 +19,7 @@ RIPS_OK, RIPS_EINVAL, RIPS_EOVERFLOW, RIPS_ENOMEM, RIPS_ECUDA = 0, -1, -2, -3, -
 
 # every symbol include/rips.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = [
-    "rips_workspace_bytes", "rips_init", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce",
+    "rips_workspace_bytes", "rips_init", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce", "rips_import_pivots",
     "rips_barcodes", "rips_filtration", "rips_apparent_pairs", "rips_nonapparent", "rips_pivots",
     "rips_pivot_lookup", "rips_stats", "rips_timings", "rips_device_bytes", "rips_kernel_launches",
     "rips_sort_u64", "rips_strerror", "rips_last_error", "rips_free",
@@ -75,6 +75,7 @@ def lib():
             getattr(l, f).argtypes = [vp, i32, pp, pi64]
         for f in ("rips_filtration", "rips_apparent_pairs", "rips_nonapparent", "rips_pivots"):
             getattr(l, f).argtypes = [vp, i32, pp, pp, pi64]
+        l.rips_import_pivots.argtypes = [vp, i32, vp, vp, i64]
         l.rips_pivot_lookup.argtypes = [vp, i32, vp, i64, vp]
         l.rips_stats.argtypes = [vp, i32, C.POINTER(RipsStats)]
         l.rips_timings.argtypes = [vp, i32, C.POINTER(RipsTimings)]
@@ -187,6 +188,14 @@ class Rips:
 
     def reduce(self, d):
         _check(lib().rips_reduce(self._h, d), "rips_reduce")
+
+    def import_pivots(self, d, t, s):
+        """Install pivots found elsewhere (host arrays, ascending by t) as dimension d's non-apparent pivots."""
+        t = np.ascontiguousarray(t, dtype=np.uint64)
+        s = np.ascontiguousarray(s, dtype=np.uint64)
+        assert t.size == s.size
+        _check(lib().rips_import_pivots(self._h, d, t.ctypes.data if t.size else None,
+                                        s.ctypes.data if s.size else None, t.size), "rips_import_pivots")
 
     # -- results
     def barcodes(self, d):
