@@ -351,6 +351,7 @@ def run_b200(args):
         tim = {d: h.timings(d) for d in range(0, D + 1)}
         parts = {"dim0_ms": tim[0]["dim0_ms"],
                  "hot_path_ms": sum(tim[d]["stage1_ms"] + tim[d]["stage2_ms"] for d in range(1, D + 1)),
+                 "reduce_device_ms": sum(tim[d]["reduce_device_ms"] for d in range(1, D + 1)),
                  "reduce_host_ms": sum(tim[d]["reduce_host_ms"] for d in range(1, D + 1)),
                  "reduce_xfer_ms": sum(tim[d]["reduce_xfer_ms"] for d in range(1, D + 1)),
                  "bars": {str(d): int(b.shape[0]) for d, b in enumerate(bars)}}

@@ -88,7 +88,8 @@ typedef struct {
     float stage1_ms;         /* whole stage 1 as enqueued (including memsets, scalar read-back) */
     float stage2_ms;         /* whole stage 2 */
     float dim0_ms;           /* d == 0 only: edge sort is part of rips_init; this is the union-find kernel */
-    float reduce_host_ms;    /* NOT hot path: serial reduction of non-apparent columns on the host */
+    float reduce_device_ms;  /* NOT hot path: non-apparent columns reduced against the apparent ones on the device */
+    float reduce_host_ms;    /* NOT hot path: serial remainder (conflicts between non-apparent columns) on the host */
     float reduce_xfer_ms;    /* NOT hot path: D2H/H2D copies around the host reduction */
 } rips_timings_t;
 

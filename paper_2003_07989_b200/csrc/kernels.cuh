@@ -111,3 +111,19 @@ cudaError_t launch_merge_ts(const u64* t1, const u64* s1, i64 n1, const u64* t2,
                             cudaStream_t st);
 cudaError_t launch_pivot_lookup(int M, const PairLayers& L, BinomTable bt, int n, const u64* red_t, const u64* red_s,
                                 i64 n2, const u64* query, i64 m, i64* s_out, cudaStream_t st);
+
+// ------------------------------------------------------------------ reduce.cu (not the hot path)
+struct PreReduceParams {
+    const u64* cols;      // non-apparent column records, coboundary order
+    i64 ncols;
+    const void* Kf;
+    int pitch, n;
+    BinomTable bt;
+    int vbits, tbits;
+    u32 thr_key;          // cofacets with key < thr_key are above the threshold
+    PairLayers layers;    // apparent pairs of this dimension
+    u32 max_additions;    // columns needing more are left to the host
+    u64* pivot_out;       // per column: 0 = reduced to zero, ~0 = left to the host, else (key << tbits | cidx(t)) + 1
+    u32* adds_out;        // per column: additions performed
+};
+cudaError_t launch_prereduce(int M, int kf_u16, const PreReduceParams& p, cudaStream_t st);

@@ -6,6 +6,11 @@
 // PAPER.md:77-79), i.e. simply the largest packed entry.
 #include "reduce_host.h"
 
+#include <chrono>
+#include <functional>
+#include <cstdio>
+#include <cstdlib>
+
 #include <queue>
 #include <unordered_map>
 
@@ -120,19 +125,98 @@ bool pop_pivot(Heap& h, uint64_t* piv)
 
 } // namespace
 
+// Oblivious column reduction (Algorithm 2) of the columns in coboundary order.  A
+// column the device has already reduced against the apparent columns (in.pre) and whose pivot no
+// earlier column owns is final at once; the others -- the conflicts between non-apparent columns, a
+// fraction of a per cent of the columns at the paper-shaped workloads -- are reduced here, a heap as
+// the working column, adding D_{lookup[low]} whether the pivot's owner is an apparent column or one
+// reduced earlier (Lemma 3: same result as adding R_i).
 void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
 {
     Ctx cx(in);
     const uint64_t cmask = (in.cbits >= 64) ? ~0ull : ((1ull << in.cbits) - 1ull);
     const uint64_t tmask = (1ull << in.tbits) - 1ull;
-    std::unordered_map<uint64_t, uint64_t> found; // second layer: t -> s for pivots found here
-    found.reserve((size_t)in.ncols * 2 + 16);
+    typedef std::priority_queue<uint64_t, std::vector<uint64_t>> Heap;
+    std::unordered_map<uint64_t, uint64_t> owner; // second layer: t -> cidx(s) of the column that owns the pivot
+    owner.reserve((size_t)in.ncols * 2 + 16);
+    auto finalize = [&](int64_t j, uint64_t piv, uint64_t cidx_s, uint32_t key_s) {
+        owner.emplace(piv & tmask, cidx_s);
+        out.piv_t.push_back(piv & tmask);
+        out.piv_s.push_back(cidx_s);
+        out.piv_key_t.push_back((uint32_t)(piv >> in.tbits));
+        out.piv_key_s.push_back(key_s);
+        out.piv_col.push_back(j);
+    };
+    // Reduction-matrix technique for the rare column on which the oblivious form runs
+    // away (it re-adds, pivot by pivot, every column an owner's reduction had added): V_i = the columns
+    // whose coboundaries sum to R_i, kept per reduced column, so that adding R_i is one step and the
+    // additions cancel in V over Z/2.  V of a column that was reduced obliviously (or on the device) is
+    // recomputed on demand by reducing it again this way; a pivot owned by a later column cannot come up
+    // while doing so, because the earlier column would have claimed it.
+    std::unordered_map<uint64_t, std::vector<uint64_t>> vstore; // cidx(s) of a reduced column -> V (cidx of columns)
+    int64_t n_vmode = 0;
+    std::function<const std::vector<uint64_t>&(uint64_t, uint64_t*)> reduce_v =
+        [&](uint64_t cidx_s, uint64_t* piv_out) -> const std::vector<uint64_t>& {
+        Heap h;
+        std::unordered_map<uint64_t, int> par; // column -> parity in V
+        auto add_col = [&](uint64_t c) { cx.push_coboundary(h, c); par[c] ^= 1; };
+        add_col(cidx_s);
+        uint64_t piv = 0;
+        bool zero = true;
+        for (;;) {
+            if (!pop_pivot(h, &piv)) break;
+            const uint64_t t = piv & tmask;
+            auto it = owner.find(t);
+            if (it != owner.end() && it->second == cidx_s) { zero = false; break; } // its own, already known pivot
+            uint64_t s2 = 0;
+            if (it != owner.end()) {
+                const uint64_t own = it->second;
+                auto vs = vstore.find(own);
+                h.push(piv);
+                if (vs == vstore.end()) {
+                    uint64_t dummy;
+                    const std::vector<uint64_t>& v = reduce_v(own, &dummy);
+                    std::vector<uint64_t> copy(v); // reduce_v may rehash vstore
+                    for (uint64_t c : copy) add_col(c);
+                } else {
+                    std::vector<uint64_t> copy(vs->second);
+                    for (uint64_t c : copy) add_col(c);
+                }
+                ++out.additions;
+                continue;
+            }
+            if (cx.apparent_lookup(t, &s2)) { h.push(piv); add_col(s2); ++out.additions; continue; }
+            zero = false;
+            break; // a new pivot
+        }
+        if (piv_out) *piv_out = zero ? ~0ull : piv;
+        std::vector<uint64_t> v;
+        for (auto& kv : par) if (kv.second) v.push_back(kv.first);
+        return vstore[cidx_s] = std::move(v);
+    };
+    const int64_t oblivious_budget = 256; // additions before a column is restarted with the V technique
+    int64_t n_fast = 0, n_slow = 0, n_def = 0, n_own_adds = 0;
     std::vector<uint64_t> store;
     for (int64_t j = 0; j < in.ncols; ++j) {
         const uint64_t cidx_s = in.cols[j] & cmask;
         const uint32_t key_s = (uint32_t)(in.cols[j] >> in.cbits);
+        if (in.pre && in.pre[j] == ~0ull) ++n_def;
+        if (in.pre && in.pre[j] != ~0ull) {
+            if (in.pre[j] == 0) {
+                out.ess_s.push_back(cidx_s);
+                out.ess_key.push_back(key_s);
+                out.ess_col.push_back(j);
+                continue;
+            }
+            const uint64_t piv = in.pre[j] - 1;
+            ++out.lookups;
+            if (owner.find(piv & tmask) == owner.end()) { finalize(j, piv, cidx_s, key_s); ++n_fast; continue; }
+        }
+        ++n_slow;
+        const int64_t adds0 = out.additions;
+        const auto tc0 = std::chrono::steady_clock::now();
         store.clear();
-        std::priority_queue<uint64_t, std::vector<uint64_t>> h(std::less<uint64_t>(), std::move(store));
+        Heap h(std::less<uint64_t>(), std::move(store));
         cx.push_coboundary(h, cidx_s);
         for (;;) {
             uint64_t piv;
@@ -146,21 +230,36 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
             uint64_t s2 = 0;
             bool hit = false;
             ++out.lookups;
-            auto it = found.find(t);
-            if (it != found.end()) { hit = true; s2 = it->second; }
+            auto it = owner.find(t);
+            if (it != owner.end()) { hit = true; s2 = it->second; }
             else hit = cx.apparent_lookup(t, &s2);
-            if (!hit) {
-                found.emplace(t, cidx_s);
-                out.piv_t.push_back(t);
-                out.piv_s.push_back(cidx_s);
-                out.piv_key_t.push_back((uint32_t)(piv >> in.tbits));
-                out.piv_key_s.push_back(key_s);
-                out.piv_col.push_back(j);
+            if (!hit) { finalize(j, piv, cidx_s, key_s); break; }
+            if (it != owner.end()) ++n_own_adds;
+            if (out.additions - adds0 >= oblivious_budget) { // runaway: start over with the V technique
+                out.additions = adds0;
+                ++n_vmode;
+                uint64_t pv = 0;
+                reduce_v(cidx_s, &pv);
+                if (pv == ~0ull) {
+                    out.ess_s.push_back(cidx_s);
+                    out.ess_key.push_back(key_s);
+                    out.ess_col.push_back(j);
+                } else
+                    finalize(j, pv, cidx_s, key_s);
                 break;
             }
             h.push(piv); // the column of s2 contains t as well: the two cancel
             cx.push_coboundary(h, s2);
             ++out.additions;
         }
+        {
+            double ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - tc0).count();
+            if (getenv("RIPS_DEBUG") && ms > 20.0)
+                fprintf(stderr, "  slow column %lld: %.1f ms, %lld additions, heap %zu, pre %llx\n", (long long)j, ms,
+                        (long long)(out.additions - adds0), h.size(), (unsigned long long)(in.pre ? in.pre[j] : 0));
+        }
     }
+    if (getenv("RIPS_DEBUG"))
+        fprintf(stderr, "host_reduce d=%d: cols %lld final at once %lld reduced here %lld (not pre-reduced %lld), additions of reduced columns %lld, restarted with V %lld\n", in.d,
+                (long long)in.ncols, (long long)n_fast, (long long)n_slow, (long long)n_def, (long long)n_own_adds, (long long)n_vmode);
 }

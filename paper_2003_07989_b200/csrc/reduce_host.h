@@ -14,7 +14,9 @@ struct HostReduceIn {
     const uint64_t* cols;     // packed column records of the non-apparent columns, coboundary order
     int64_t ncols;
     int cbits;
-    int tbits;                // bits of C(n, d+2) - 1
+    int tbits;                // bits of the row index field
+    const uint64_t* pre;      // per column, from the device pre-reduction against the apparent columns: 0 = zero column,
+                              // ~0 = not pre-reduced, else (key << tbits | cidx(t)) + 1 with t not an apparent row; may be NULL
 };
 
 struct HostReduceOut {

@@ -58,7 +58,7 @@ struct DimState {
     int compact = 0;
     // stage 1: column records (sorted), pair slots (unsorted until stage 2), the two small lists
     bool have_s1 = false;
-    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch;
+    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch, pre_piv, pre_adds;
     u64* cols = nullptr; // sorted packed column records (points into colsA or colsB)
     i64 len = 0;         // columns
     i64 slots = 0;       // records in the column / pair arrays (len in compact mode, else C(n,d+1) with sentinels)
@@ -525,11 +525,39 @@ int run_reduce(rips_ctx* c, int d)
     s.have_red = false;
     invalidate_views(s, false, false, false, true);
     s.bars.clear();
-    s.tim.reduce_host_ms = s.tim.reduce_xfer_ms = 0.f;
+    s.tim.reduce_host_ms = s.tim.reduce_xfer_ms = s.tim.reduce_device_ms = 0.f;
     HostReduceOut out;
     if (s.n_non > 0) {
+        // ---- device: every non-apparent column reduced against the apparent columns (reduce.cu)
+        std::vector<u64> h_pre((size_t)s.n_non);
+        std::vector<u32> h_adds((size_t)s.n_non);
+        {
+            double td = now_ms();
+            RC(ensure(c, s.pre_piv, (size_t)s.n_non * 8));
+            RC(ensure(c, s.pre_adds, (size_t)s.n_non * 4));
+            PreReduceParams pp;
+            pp.cols = s.non;
+            pp.ncols = s.n_non;
+            pp.Kf = c->d_Kf;
+            pp.pitch = c->kf_pitch;
+            pp.n = (int)c->n;
+            pp.bt = c->bt();
+            pp.vbits = c->vbits;
+            pp.tbits = s.tbits;
+            pp.thr_key = c->thr_key;
+            pp.layers = layers_of(s);
+            pp.max_additions = 64;
+            pp.pivot_out = (u64*)s.pre_piv.p;
+            pp.adds_out = (u32*)s.pre_adds.p;
+            CU(launch_prereduce(s.M, c->kf_u16, pp, c->stream));
+            c->launches += 1;
+            CU(cudaMemcpyAsync(h_pre.data(), s.pre_piv.p, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaMemcpyAsync(h_adds.data(), s.pre_adds.p, (size_t)s.n_non * 4, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+            s.tim.reduce_device_ms = (float)(now_ms() - td);
+            for (u32 a : h_adds) out.additions += a;
+        }
         double t0 = now_ms();
-        CU(cudaStreamSynchronize(c->stream));
         if (c->h_K.empty() && c->E) {
             c->h_K.resize((size_t)c->E);
             CU(cudaMemcpy(c->h_K.data(), c->d_K, (size_t)c->E * 4, cudaMemcpyDeviceToHost));
@@ -556,6 +584,7 @@ int run_reduce(rips_ctx* c, int d)
         in.ncols = s.n_non;
         in.cbits = s.cbits;
         in.tbits = s.tbits;
+        in.pre = h_pre.data();
         host_reduce_columns(in, out);
         double t2 = now_ms();
         s.tim.reduce_host_ms = (float)(t2 - t1);
@@ -613,7 +642,7 @@ int check_dim(rips_ctx* c, int d, int lo)
 void free_dim(rips_ctx* c, DimState& s)
 {
     DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.pairsA, &s.pairsB, &s.irrA, &s.irrB, &s.nonA, &s.nonB,
-                     &s.pair_scratch, &s.red_t,
+                     &s.pair_scratch, &s.pre_piv, &s.pre_adds, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
     if (s.ev_made) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(s.ev[i]);

@@ -44,14 +44,6 @@ __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int 
     return lo < n && (__ldg(a + lo) >> shift) == x;
 }
 
-// append `val` to a global list with capacity `cap`; the counter keeps counting past the capacity
-__device__ __forceinline__ void list_append(u64* list, u64 cap, u64* counter, u64 val)
-{
-    u64 pos = atomicAdd((unsigned long long*)counter, 1ull);
-    if (pos < cap) list[pos] = val;
-}
-
-
 // shared-memory digit histograms of one block
 struct BlockHists {
     u32 (*cols)[256];   // [S1_MAX_FUSED][256]

@@ -39,7 +39,7 @@ class RipsStats(C.Structure):
 class RipsTimings(C.Structure):
     _fields_ = [(k, C.c_float) for k in (
         "clear_bitmap_ms", "enumerate_ms", "sort_hist_ms", "sort_pass_ms", "apparent_ms", "pair_hist_ms",
-        "pair_sort_ms", "stage1_ms", "stage2_ms", "dim0_ms", "reduce_host_ms", "reduce_xfer_ms")]
+        "pair_sort_ms", "stage1_ms", "stage2_ms", "dim0_ms", "reduce_device_ms", "reduce_host_ms", "reduce_xfer_ms")]
 
     def as_dict(self):
         return {k: float(getattr(self, k)) for k, _ in self._fields_}
