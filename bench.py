@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-scale-row", action="store_true",
+                    help="skip the scale row (stage 1 + 2 at d = dim_max+1: the C(n, dim_max+2) simplices the config names)")
     ap.add_argument("--warmup-seconds", type=float, default=0.6,
                     help="keep warming up until this much time has passed (gives the clock sampler load to see)")
     return ap.parse_args()
@@ -362,6 +364,35 @@ def run_b200(args):
            "h2d_bytes_per_step": int(host.numel() * 4), "d2h_bytes_per_step": int(d2h_bytes),
            "what": "rips_init(host matrix) + rips_compute + rips_barcodes(host) + rips_free"}
 
+    # ---- scale row: the same kernels one dimension up, on the simplices the config names
+    scale = None
+    if not args.no_scale_row and D + 1 <= 4:
+        need = 5 * 8 * comb(w.n, D + 2) + (1 << 30)
+        free_b, _ = torch.cuda.mem_get_info()
+        if need < free_b:
+            reps = []
+            for _ in range(3):
+                barrier()
+                e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                e0.record(); g.stage1(D + 1); e1.record(); g.stage2(D + 1); e2.record()
+                torch.cuda.synchronize()
+                reps.append((e0.elapsed_time(e1), e1.elapsed_time(e2), g.timings(D + 1)))
+            s1, s2, tm = min(reps, key=lambda r: r[0] + r[1])
+            st = g.stats(D + 1)
+            nbytes = 2 * RECORD_BYTES * st["n_slots"]
+            scale = {"what": f"rips_stage1({D + 1}) + rips_stage2({D + 1}) with the pivots of dimension {D} as the clearing set",
+                     "candidates": st["n_candidates"], "columns": st["n_columns"], "apparent": st["n_apparent"],
+                     "stage1_ms": s1, "stage2_ms": s2,
+                     "simplices_per_s": world * st["n_candidates"] / ((ranks.max_over_ranks(s1 + s2)) * 1e-3),
+                     "fused_kernel_ms": tm["enumerate_ms"], "fused_kernel_gbs": (nbytes + st["n_candidates"] / 8) / tm["enumerate_ms"] / 1e6,
+                     "filtration_sort_pass_ms": tm["sort_pass_ms"] / max(1, st["sort_passes"]),
+                     "filtration_sort_pass_gbs": nbytes / (tm["sort_pass_ms"] / max(1, st["sort_passes"])) / 1e6,
+                     "pair_partition_pass_ms": tm["pair_sort_ms"] / max(1, st["pair_sort_passes"]),
+                     "pair_partition_pass_gbs": nbytes / (tm["pair_sort_ms"] / max(1, st["pair_sort_passes"])) / 1e6,
+                     "hbm_bytes": 4 * nbytes + st["n_candidates"] / 8,
+                     "overall_gbs": (4 * nbytes + st["n_candidates"] / 8) / (s1 + s2) / 1e6,
+                     "device_bytes": g.device_bytes()}
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         s, t, cores, desc, _ = oracle_sample(w, args.cpu_seconds)
@@ -373,7 +404,7 @@ def run_b200(args):
                 "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
                 "config": workload_dict(w, n_cand), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                 "roofline": roofline, "cpu_baseline": cpu,
-                "kernels": kernels,
+                "kernels": kernels, "scale_row": scale,
                 "barcode": {"end_to_end_ms": e2e_t, "first_compute_ms": first_compute_ms, **(parts or {})},
                 "stats": {str(d): {k: stats[d][k] for k in ("n_candidates", "n_columns", "n_cleared",
                                                             "n_removed_by_diameter", "n_apparent", "n_regular",

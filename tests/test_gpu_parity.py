@@ -142,3 +142,28 @@ def test_invalid_inputs(R):
     with R.Rips(neg0, 3, 1) as h:
         h.compute()
         assert np.array_equal(h.barcodes(0), oracle.barcodes(np.abs(neg0), 3, 1)[0]["bars"].reshape(-1, 2))
+
+
+def test_scale_row_entry_points(R):
+    """rips_stage1 / rips_stage2 at d = dim_max + 1 (the scale row): the same
+    arrays the oracle produces for that dimension."""
+    w = inputs.config(2, 36)
+    o = oracle.barcodes(w.dist, w.n, 3, w.threshold)
+    with R.Rips(w.dist, w.n, 2, w.threshold) as g:
+        g.compute()
+        g.stage1(3)
+        g.stage2(3)
+        fd, fc = g.filtration(3)
+        assert np.array_equal(_np(fc).astype(np.uint64), o[3]["filt_cidx"])
+        assert np.array_equal(_np(fd).view(np.uint32), o[3]["filt_diam"].view(np.uint32))
+        at, as_ = g.apparent_pairs(3)
+        assert np.array_equal(_np(at).astype(np.uint64), o[3]["app_t"])
+        assert np.array_equal(_np(as_).astype(np.uint64), o[3]["app_s"])
+        nd, nc = g.nonapparent(3)
+        assert np.array_equal(_np(nc).astype(np.uint64), o[3]["non_cidx"])
+        st = g.stats(3)
+        assert st["n_cleared"] == o[2]["pivot_t"].size
+        # re-running the stages gives the same arrays (bench.py's step)
+        g.stage1(3); g.stage2(3)
+        at2, _ = g.apparent_pairs(3)
+        assert bool((at2 == at).all())
