@@ -92,6 +92,8 @@ struct rips_ctx {
     int dim_max = 0;
     float threshold = 0;
     cudaStream_t stream = 0;
+    cudaStream_t stream2 = nullptr; // stage 2's sorts run here, beside the filtration sort of stage 1 on `stream`
+    cudaEvent_t ev_join = nullptr;
     int kmax = 0; // binomial table holds C(v,k), k <= kmax
     std::vector<u64> h_binom;
     std::vector<float> h_values;
@@ -109,7 +111,7 @@ struct rips_ctx {
     u64* h_counters = nullptr; // pinned
     u32 n_distinct = 0, thr_key = 0;
     int key_bits = 1;
-    DevBuf sort_scratch;
+    DevBuf sort_scratch, sort_scratch2;
     // dim 0
     DevBuf d0_pairs, d0_death, d0_uf;
     std::vector<DimState> dims; // index d, 0 .. dim_max+1
@@ -142,13 +144,13 @@ void release(rips_ctx* c, DevBuf& b)
     b.cap = 0;
 }
 
-void ev_record(rips_ctx* c, DimState& s, int which)
+void ev_record(rips_ctx* c, DimState& s, int which, cudaStream_t st = nullptr)
 {
     if (!s.ev_made) {
         for (int i = 0; i < EV_COUNT; ++i) { cudaEventCreate(&s.ev[i]); s.ev_rec[i] = false; }
         s.ev_made = true;
     }
-    cudaEventRecord(s.ev[which], c->stream);
+    cudaEventRecord(s.ev[which], st ? st : c->stream);
     s.ev_rec[which] = true;
 }
 float ev_ms(DimState& s, int a, int b)
@@ -398,8 +400,9 @@ int run_stage1(rips_ctx* c, int d)
     s.pair_plan = sort_make_plan(s.tbits, s.tbits + pvbits);
     RC(ensure(c, c->sort_scratch, sort_scratch_bytes((i64)cap, plan)));
     RC(ensure(c, s.pair_scratch, sort_scratch_bytes((i64)cap, s.pair_plan)));
-    const bool fused = plan.npasses <= 3;           // S1_MAX_FUSED digits
-    s.pair_fused = s.pair_plan.npasses <= 2;        // S1_MAX_FUSED_P digits
+    static const int nofuse = getenv("RIPS_NO_FUSED_HIST") ? atoi(getenv("RIPS_NO_FUSED_HIST")) : 0; // tuning: bit 0 columns, bit 1 pairs
+    const bool fused = plan.npasses <= 3 && !(nofuse & 1);           // S1_MAX_FUSED digits
+    s.pair_fused = s.pair_plan.npasses <= 2 && !(nofuse & 2);        // S1_MAX_FUSED_P digits
     // provisioned for (d+1)/n of the columns to hold the top vertices (those pairs are irregular) and as many
     // non-apparent ones; a run that needs more is repeated once with the exact sizes
     u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 8));
@@ -478,25 +481,28 @@ int run_stage2(rips_ctx* c, int d)
     if (s.have_s2 && !s.pairs_fresh) return RIPS_OK; // nothing new to partition: the pair store is current
     s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
-    ev_record(c, s, EV_S2_BEGIN);
+    // Everything below runs on the second stream: it only needs the fused kernel's outputs (complete: stage 1
+    // read its counters back), so it overlaps the filtration sort that stage 1 left running on the main stream.
+    cudaStream_t st2 = c->stream2 ? c->stream2 : c->stream;
+    ev_record(c, s, EV_S2_BEGIN, st2);
     // ---- a8: the two small out-of-order lists: irregular pairs by cidx(t), non-apparent columns by
     // (key, vertices), which is the coboundary order
     {
         SortPlan pi = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
         RC(ensure(c, s.irrA, 16));
         RC(ensure(c, s.irrB, (size_t)s.n_irr * 8));
-        RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_irr, pi)));
+        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(s.n_irr, pi)));
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, s.n_irr, pi, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, s.n_irr, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches));
         s.irr = res;
         SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
         RC(ensure(c, s.nonA, 16));
         RC(ensure(c, s.nonB, (size_t)s.n_non * 8));
-        RC(ensure(c, c->sort_scratch, sort_scratch_bytes(s.n_non, pn)));
-        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(s.n_non, pn)));
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch2.p, st2, &res, nullptr, &c->launches));
         s.non = res;
     }
-    ev_record(c, s, EV_S2_APP);
+    ev_record(c, s, EV_S2_APP, st2);
     // ---- a9: stable partition of the pair slots by the cofacet vertex v: the regular pairs come out
     // ascending by cidx(t), the sentinels (v = n) behind them
     s.stats.pair_sort_passes = s.slots > 1 ? s.pair_plan.npasses : 0;
@@ -507,10 +513,14 @@ int run_stage2(rips_ctx* c, int d)
     st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
     s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
     u64* res = nullptr;
-    CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, c->stream, &res, &st,
+    CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, st2, &res, &st,
                 &c->launches, s.pair_fused, true));
     s.reg = res;
-    ev_record(c, s, EV_S2_END);
+    ev_record(c, s, EV_S2_END, st2);
+    if (st2 != c->stream) { // join: whatever follows on the main stream sees stage 2's results
+        CU(cudaEventRecord(c->ev_join, st2));
+        CU(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+    }
     s.pairs_fresh = false;
     s.have_s2 = true;
     return RIPS_OK;
@@ -788,6 +798,10 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     c->threshold = threshold;
     c->stream = (cudaStream_t)stream;
     c->kmax = dim_max + 3;
+    if (!getenv("RIPS_ONE_STREAM")) {
+        if (cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream2 = nullptr; }
+    }
+    if (cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join = nullptr; c->stream2 = nullptr; }
     if (const char* e = getenv("RIPS_FAST_VISITS")) c->fast_visits = atoi(e);
     build_binom(n, c->kmax, c->h_binom);
     if (hbinom(c, n, dim_max + 2) >> 62) { delete c; return RIPS_EOVERFLOW; }
@@ -808,8 +822,11 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
 void rips_free(rips_ctx* c)
 {
     if (!c) return;
+    if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
     for (DimState& s : c->dims) free_dim(c, s);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     release(c, c->sort_scratch);
+    release(c, c->sort_scratch2);
     release(c, c->d0_pairs);
     release(c, c->d0_death);
     release(c, c->d0_uf);

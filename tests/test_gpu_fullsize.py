@@ -144,3 +144,36 @@ def test_config2_lower_dimensions_complete(R):
             assert np.array_equal(pt.cpu().numpy().astype(np.uint64), o[d]["pivot_t"])
             assert np.array_equal(ps.cpu().numpy().astype(np.uint64), o[d]["pivot_s"])
             assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32))
+
+
+def test_second_workload_dim1_random_permutation_matrix(R):
+    """SURVEY.md 8(f) item 4, the experiment of PAPER.md:719-729: dimension-1 apparent pairs of a uniformly
+    random permutation matrix.  (a) the apparent fraction against the closed form behind the paper's printed
+    means (pin P11; the paper reports a very low variance); (b) on a slice of the edges, the exact arrays
+    against the oracle."""
+    import math
+    import torch
+    n = 3000
+    low = inputs.permutation_matrix_lower(n, 7)
+    E = n * (n - 1) // 2
+    with R.Rips(torch.from_numpy(low).cuda(), n, 1) as g:
+        g.dim0()
+        g.stage1(1)
+        g.stage2(1)
+        st = g.stats(1)
+        assert st["n_candidates"] == E and st["n_cleared"] == n - 1 and st["n_columns"] == E - (n - 1)
+        closed = 1 - (math.sqrt(math.pi) / 2) * math.exp(math.lgamma(n - 1) - math.lgamma(n - 0.5))
+        assert abs(st["n_apparent"] / E - closed) < 1e-3
+        z = oracle.dim0(low, n)
+        lo, hi = E // 2, E // 2 + 20000
+        od, oc, _ = oracle.stage1(low, n, 1, inf, z["t"], lo, hi, sort=False)
+        s2 = oracle.stage2(low, n, 1, od, oc)
+        at, as_ = g.apparent_pairs(1)
+        m = (as_ >= lo) & (as_ < hi)
+        gs, order = torch.sort(as_[m])
+        o_order = np.argsort(s2["app_s"], kind="stable")
+        assert np.array_equal(gs.cpu().numpy().astype(np.uint64), s2["app_s"][o_order])
+        assert np.array_equal(at[m][order].cpu().numpy().astype(np.uint64), s2["app_t"][o_order])
+        nd, nc = g.nonapparent(1)
+        m = (nc >= lo) & (nc < hi)
+        assert np.array_equal(torch.sort(nc[m])[0].cpu().numpy().astype(np.uint64), np.sort(s2["non_cidx"]))
