@@ -9,11 +9,11 @@
 
 namespace {
 
-constexpr int SORT_THREADS = 512;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
+constexpr int SORT_THREADS = 384;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
 constexpr int SORT_IPT = 12;
-constexpr int SORT_MIN_BLOCKS = 2;
+constexpr int SORT_MIN_BLOCKS = 3;
 constexpr int SORT_LB_BATCH = 8;     // predecessor tiles read per look-back step
-constexpr int SORT_RANK_BATCH = 6;   // records ranked per pipelined batch (divides SORT_IPT)
+constexpr int SORT_RANK_BATCH = 3;   // records ranked per pipelined batch (divides SORT_IPT)
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 
