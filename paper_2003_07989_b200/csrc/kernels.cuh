@@ -86,7 +86,7 @@ struct Stage1Params {
     FusedHist fh_cols;   // digit histogram of the filtration sort (over every slot written to cols_out)
     FusedHist fh_pairs;  // digit histogram of the partition of pairs_out by v
 };
-int stage1_chunk(u64 total);
+int stage1_chunk(u64 total, int compact);
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
 // bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask
 cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st);

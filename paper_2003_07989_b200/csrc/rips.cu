@@ -93,7 +93,8 @@ struct rips_ctx {
     float threshold = 0;
     cudaStream_t stream = 0;
     cudaStream_t stream2 = nullptr; // stage 2's sorts run here, beside the filtration sort of stage 1 on `stream`
-    cudaEvent_t ev_join = nullptr;
+    cudaStream_t stream3 = nullptr; // the sort of the non-apparent columns, beside the other two
+    cudaEvent_t ev_join = nullptr, ev_join3 = nullptr, ev_fused = nullptr;
     int kmax = 0; // binomial table holds C(v,k), k <= kmax
     std::vector<u64> h_binom;
     std::vector<float> h_values;
@@ -111,7 +112,7 @@ struct rips_ctx {
     u64* h_counters = nullptr; // pinned
     u32 n_distinct = 0, thr_key = 0;
     int key_bits = 1;
-    DevBuf sort_scratch, sort_scratch2;
+    DevBuf sort_scratch, sort_scratch2, sort_scratch3;
     // dim 0
     DevBuf d0_pairs, d0_death, d0_uf;
     std::vector<DimState> dims; // index d, 0 .. dim_max+1
@@ -346,7 +347,7 @@ int run_stage1(rips_ctx* c, int d)
     // q of admissible edges (q^(edges of the simplex)) and compact when most are dropped
     const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
     s.compact = (c->thr_key != 0 && std::pow(q, (double)(s.M * (s.M - 1) / 2)) < 0.5) ? 1 : 0;
-    const int chunk = stage1_chunk(s.total);
+    const int chunk = stage1_chunk(s.total, s.compact);
     const i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
     Stage1Params p;
     p.Kf = c->d_Kf;
@@ -407,6 +408,22 @@ int run_stage1(rips_ctx* c, int d)
     // non-apparent ones; a run that needs more is repeated once with the exact sizes
     u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 8));
     u64 non_cap = std::max<u64>(s.nonA.cap / 8, std::max<u64>(4096, cap / 8));
+    // a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys, and the
+    // sentinels of the dropped candidates (largest key) end up behind the len columns
+    bool sorted_early = false;
+    auto enqueue_a6 = [&](u64 nrec) -> int {
+        SortTimes st;
+        st.enabled = true;
+        if (!s.ev_made) ev_record(c, s, EV_S1_SORTBEG);
+        st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
+        s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
+        u64* res = nullptr;
+        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, (i64)nrec, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches,
+                    fused));
+        s.cols = res;
+        ev_record(c, s, EV_S1_END);
+        return RIPS_OK;
+    };
     for (int attempt = 0;; ++attempt) {
         RC(ensure(c, s.irrA, (size_t)irr_cap * 8));
         RC(ensure(c, s.nonA, (size_t)non_cap * 8));
@@ -435,10 +452,23 @@ int run_stage1(rips_ctx* c, int d)
         CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
         c->launches += 1;
         ev_record(c, s, EV_S1_ENUM);
-        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
+        if (!s.compact && c->stream2) {
+            // slot mode: the number of records is known, so the filtration sort is enqueued at once and
+            // the counters come back over the second stream while it runs
+            CU(cudaEventRecord(c->ev_fused, c->stream));
+            RC(ensure(c, s.colsB, (size_t)cap * 8));
+            RC(enqueue_a6(cap));
+            sorted_early = true;
+            CU(cudaStreamWaitEvent(c->stream2, c->ev_fused, 0));
+            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream2));
+            CU(cudaStreamSynchronize(c->stream2));
+        } else {
+            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaStreamSynchronize(c->stream));
+        }
         const u64 ni = c->h_counters[S1C_IRREGULAR], nn = c->h_counters[S1C_NONAPP];
         if (ni <= irr_cap && nn <= non_cap) break;
+        if (sorted_early) { CU(cudaStreamSynchronize(c->stream)); sorted_early = false; }
         if (attempt >= 1) { g_last_error = "rips_stage1: list capacities still too small on the second attempt"; return RIPS_ECUDA; }
         irr_cap = std::max(irr_cap, ni); // rare: more irregular pairs / non-apparent columns than provisioned; run again
         non_cap = std::max(non_cap, nn);
@@ -455,18 +485,11 @@ int run_stage1(rips_ctx* c, int d)
     s.stats.n_nonapparent = s.n_non;
     s.stats.n_slots = s.slots;
     s.stats.n_regular = s.n_reg;
-    // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys,
-    // and the sentinels of the dropped candidates (largest key) end up behind the len columns
     s.stats.sort_passes = s.slots > 1 ? plan.npasses : 0;
-    RC(ensure(c, s.colsB, (size_t)s.slots * 8));
-    SortTimes st;
-    st.enabled = true;
-    st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
-    s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
-    u64* res = nullptr;
-    CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, s.slots, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
-    s.cols = res;
-    ev_record(c, s, EV_S1_END);
+    if (!sorted_early) {
+        RC(ensure(c, s.colsB, (size_t)s.slots * 8));
+        RC(enqueue_a6((u64)s.slots));
+    }
     s.have_s1 = true;
     s.pairs_fresh = true;
     return RIPS_OK;
@@ -498,8 +521,13 @@ int run_stage2(rips_ctx* c, int d)
         SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
         RC(ensure(c, s.nonA, 16));
         RC(ensure(c, s.nonB, (size_t)s.n_non * 8));
-        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(s.n_non, pn)));
-        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch2.p, st2, &res, nullptr, &c->launches));
+        cudaStream_t st3 = (c->stream3 && st2 != c->stream) ? c->stream3 : st2;
+        RC(ensure(c, c->sort_scratch3, sort_scratch_bytes(s.n_non, pn)));
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches));
+        if (st3 != st2) { // join the third stream into the second
+            CU(cudaEventRecord(c->ev_join3, st3));
+            CU(cudaStreamWaitEvent(st2, c->ev_join3, 0));
+        }
         s.non = res;
     }
     ev_record(c, s, EV_S2_APP, st2);
@@ -800,7 +828,10 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     c->kmax = dim_max + 3;
     if (!getenv("RIPS_ONE_STREAM")) {
         if (cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream2 = nullptr; }
+        if (cudaStreamCreateWithFlags(&c->stream3, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream3 = nullptr; }
+        if (cudaEventCreateWithFlags(&c->ev_join3, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join3 = nullptr; c->stream3 = nullptr; }
     }
+    if (cudaEventCreateWithFlags(&c->ev_fused, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_fused = nullptr; c->stream2 = nullptr; }
     if (cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join = nullptr; c->stream2 = nullptr; }
     if (const char* e = getenv("RIPS_FAST_VISITS")) c->fast_visits = atoi(e);
     build_binom(n, c->kmax, c->h_binom);
@@ -822,11 +853,15 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
 void rips_free(rips_ctx* c)
 {
     if (!c) return;
+    if (c->stream3) { cudaStreamSynchronize(c->stream3); cudaStreamDestroy(c->stream3); }
+    if (c->ev_join3) cudaEventDestroy(c->ev_join3);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
     for (DimState& s : c->dims) free_dim(c, s);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_fused) cudaEventDestroy(c->ev_fused);
     release(c, c->sort_scratch);
     release(c, c->sort_scratch2);
+    release(c, c->sort_scratch3);
     release(c, c->d0_pairs);
     release(c, c->d0_death);
     release(c, c->d0_uf);

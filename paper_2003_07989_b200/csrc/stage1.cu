@@ -21,12 +21,14 @@
 //     coalesced stores.  With a threshold survivors are compacted in increasing index with a
 //     warp-level decoupled look-back.
 //   * the digit histograms of the two sorts that follow are accumulated on the way out.
+#include <cstdlib>
+
 #include "apparent.cuh"
 #include "kernels.cuh"
 
 namespace {
 
-constexpr int S1_THREADS = 512;
+constexpr int S1_THREADS = 1024;
 constexpr int S1_WARPS = S1_THREADS / 32;
 constexpr int S1_CHUNK = 512;          // most candidates per warp chunk (unit of work and of the look-back chain)
 constexpr int S1_MAX_FUSED = 3;        // digits of the filtration sort histogrammed on the way out
@@ -55,8 +57,11 @@ struct BlockHists {
     u32 pmk[S1_MAX_FUSED_P];
 };
 
-template <int M, typename KT>
-__global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const Stage1Params p, int k_in_smem)
+// KS: the key matrix is staged in shared memory.  A template parameter, not a run-time flag, so that the
+// compiler addresses Kf with 32-bit shared-memory addresses (LDS) instead of generic 64-bit ones: the
+// kernel is bound by instruction issue, and address arithmetic is a large part of its instructions.
+template <int M, typename KT, bool KS>
+__global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const Stage1Params p)
 {
     extern __shared__ __align__(16) unsigned char smem1[];
     __shared__ u32 s_hist_cols[S1_MAX_FUSED][256];
@@ -73,20 +78,22 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
 
     // ---- shared memory carve-up: [Kf] [staging (compact mode)]
     size_t off_b = 0;
-    const KT* Kf = reinterpret_cast<const KT*>(p.Kf);
-    if (k_in_smem) {
+    const KT* __restrict__ Kf;
+    if (KS) {
         const int cnt16 = (int)(((size_t)n * pitch * sizeof(KT) + 15) / 16); // the buffer is padded to 16 bytes
         uint4* dst = reinterpret_cast<uint4*>(smem1);
         const uint4* src = reinterpret_cast<const uint4*>(p.Kf);
         for (int i = tid; i < cnt16; i += S1_THREADS) dst[i] = __ldg(src + i);
         Kf = reinterpret_cast<const KT*>(smem1);
         off_b = (size_t)cnt16 * 16;
+    } else {
+        Kf = reinterpret_cast<const KT*>(p.Kf);
     }
     u64* stage_cols = nullptr;
     u64* stage_pairs = nullptr;
     if (compact && !count_only) {
-        stage_cols = reinterpret_cast<u64*>(smem1 + off_b) + (size_t)warp * (2 * S1_CHUNK);
-        stage_pairs = stage_cols + S1_CHUNK;
+        stage_cols = reinterpret_cast<u64*>(smem1 + off_b) + (size_t)warp * (2 * p.chunk);
+        stage_pairs = stage_cols + p.chunk;
     }
     BlockHists H;
     H.cols = s_hist_cols;
@@ -353,10 +360,11 @@ template <int M, typename KT>
 cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 {
     const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
-    const int k_in = (!p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
+    static const bool kf_global = getenv("RIPS_KF_GLOBAL") != nullptr; // tuning: never stage Kf in shared memory
+    const int k_in = (!kf_global && !p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
     const size_t smem = (k_in ? kf_bytes : 0) +
-                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * S1_CHUNK * 8 : 0);
-    auto kern = enumerate_apparent_kernel<M, KT>;
+                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.chunk * 8 : 0);
+    auto kern = k_in ? enumerate_apparent_kernel<M, KT, true> : enumerate_apparent_kernel<M, KT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) return e;
     int per_sm = 1;
@@ -367,7 +375,7 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     i64 g = (p.tiles + S1_WARPS - 1) / S1_WARPS;
     if (g > (i64)sms * per_sm) g = (i64)sms * per_sm;
-    kern<<<(unsigned)g, S1_THREADS, smem, st>>>(p, k_in);
+    kern<<<(unsigned)g, S1_THREADS, smem, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -375,11 +383,12 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 
 // Candidates per warp chunk: S1_CHUNK when there is plenty of work, less (a multiple of 32) when the
 // index space is small, so that every SM still gets warps to run.
-int stage1_chunk(u64 total)
+int stage1_chunk(u64 total, int compact)
 {
     u64 c = (total / (148ull * 64) + 31) / 32 * 32;
     if (c < 32) c = 32;
     if (c > (u64)S1_CHUNK) c = S1_CHUNK;
+    if (compact && c > 256) c = 256; // two staged records per candidate and warp must fit shared memory
     return (int)c;
 }
 
