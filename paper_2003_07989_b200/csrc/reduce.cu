@@ -108,10 +108,8 @@ __global__ void __launch_bounds__(PR_THREADS) prereduce_kernel(const PreReducePa
                 i64 p1 = lower_bound_field_d(p.layers.reg, p.layers.n_reg, 0, tmask, t);
                 if (p1 < p.layers.n_reg && (__ldg(p.layers.reg + p1) & tmask) == t) {
                     // s' = t minus its top vertex v
-                    const int v = (int)(__ldg(p.layers.reg + p1) >> p.layers.tbits);
                     int tv[M + 1];
                     decode_simplex<M + 1>(p.bt, t, p.n, tv);
-                    (void)v;
 #pragma unroll
                     for (int j = 0; j < M; ++j) s2[j] = tv[j];
                     hit = true;

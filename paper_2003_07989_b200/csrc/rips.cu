@@ -792,11 +792,14 @@ int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes)
     if (C(dim_max + 2) >> 62) return RIPS_EOVERFLOW;
     long double total = 0;
     const long double E = (long double)n * (n - 1) / 2;
-    total += E * 36 + (long double)b.size() * 8;
+    // set-up: distances, edge records (+ sort buffer), lower-triangle keys, values, full key matrix, binomials
+    total += E * 36 + (long double)n * (n + 3) * 4 + (long double)b.size() * 8;
     for (int d = 1; d <= dim_max; ++d) {
         long double cand = (long double)C(d + 1);
-        // two column buffers, pair buffers (2) + non-apparent, bitmap, look-back words, sort scratch
-        total += cand * 8 * 5 + cand / 8 + cand / 4096 * 8 * 3 + cand / 8192 * 512 * 8 + (1 << 16);
+        // slot mode: column records and pair slots, each with its ping-pong buffer (4 x 8 bytes per candidate),
+        // the two small lists with theirs (2 x 2 x cand/8 records), the clearing bitmap, look-back words of the
+        // sorts (256 words per tile of 4608 records, two sorts in flight), sort scratch heads
+        total += cand * 32 + cand * 4 + cand / 8 + cand / 4608 * 256 * 8 * 2 + (3 << 16);
     }
     if (total > 9.0e18L) return RIPS_EOVERFLOW;
     *bytes = (int64_t)total;

@@ -46,6 +46,13 @@ __device__ __forceinline__ bool in_sorted(const u64* __restrict__ a, i64 n, int 
     return lo < n && (__ldg(a + lo) >> shift) == x;
 }
 
+// a lane's pair (v1, x), x < v1, 32 positions further in the order e = C(v1, 2) + x
+__device__ __forceinline__ void lane_advance(int& v1, int& x)
+{
+    x += 32;
+    while (x >= v1) { x -= v1; ++v1; }
+}
+
 // shared-memory digit histograms of one block
 struct BlockHists {
     u32 (*cols)[256];   // [S1_MAX_FUSED][256]
@@ -130,53 +137,59 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
         int rem = (p.total - idx) < (u64)p.chunk ? (int)(p.total - idx) : p.chunk;
         int v[M];
         decode_simplex_fast<M>(p.bt, idx, n, v); // warp-uniform
-        int v0 = v[0];
         u32 wcount = 0;
-        bool new_upper = true;
-        u32 up2 = 0xffffffffu;
+        // offset of the chunk's first candidate inside its slab: a slab fixes the vertices v[M-1] > ... > v[2]
+        // (all of them for M = 2: one slab) and holds the C(v[2], 2) pairs v[1] > v[0] in index order
+        i64 e0 = (i64)v[1] * (v[1] - 1) / 2 + v[0];
 
         while (rem > 0) {
-            // ---- per row: keys among v[1..M-1], upper part of the record, the shared window of U
-            if (M > 2 && new_upper) {
-                up2 = 0xffffffffu;
+            // ---- per slab (warp-uniform): keys among v[2..M-1], upper part of the record, and the window
+            // uw[l] = min_j>=2 key1(v_j, n-1-l), the part of the cofacet test of vertex n-1-l the whole slab shares
+            u32 up2 = 0xffffffffu;
 #pragma unroll
-                for (int a = 3; a < M; ++a)
+            for (int a = 3; a < M; ++a)
 #pragma unroll
-                    for (int b = 2; b < a; ++b) up2 = min(up2, (u32)Kf[v[a] * pitch + v[b]]);
-                new_upper = false;
-            }
-            u32 up1 = up2;
+                for (int b = 2; b < a; ++b) up2 = min(up2, (u32)Kf[v[a] * pitch + v[b]]);
+            u64 slab_low = 0;
 #pragma unroll
-            for (int a = 2; a < M; ++a) up1 = min(up1, (u32)Kf[v[a] * pitch + v[1]]);
-            u64 lowbase = 0;
-#pragma unroll
-            for (int j = M - 1; j >= 1; --j) lowbase = (lowbase << vbits) | (u64)(u32)v[j];
-            lowbase <<= vbits;
-            const int vtop = v[M - 1];
-            const int row_len = min(v[1] - v0, rem);
-            // window of the row: uw[l] = min_j>=1 key1(v_j, n-1-l), the part of the cofacet test of vertex
-            // n-1-l that every column of the row shares
+            for (int j = M - 1; j >= 2; --j) slab_low = (slab_low << vbits) | (u64)(u32)v[j];
+            slab_low <<= 2 * vbits;
+            const i64 slab_len = (M > 2) ? (i64)v[M > 2 ? 2 : 1] * (v[M > 2 ? 2 : 1] - 1) / 2 : (i64)n * (n - 1) / 2;
+            const int seg = (slab_len - e0) < (i64)rem ? (int)(slab_len - e0) : rem;
             if (!count_only) {
                 __syncwarp();
                 u32 u = 0;
                 if (lane < kwin) {
                     u = 0xffffffffu;
 #pragma unroll
-                    for (int j = 1; j < M; ++j) u = min(u, (u32)Kf[v[j] * pitch + (n - 1 - lane)]);
+                    for (int j = 2; j < M; ++j) u = min(u, (u32)Kf[v[j] * pitch + (n - 1 - lane)]);
                 }
                 uw[lane] = u;
                 __syncwarp();
             }
+            // ---- this lane's first pair (v1, x) of the segment: e = C(v1, 2) + x
+            int v1, x;
+            {
+                const i64 e = e0 + lane;
+                v1 = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)e)) * 0.5f);
+                if (v1 < 1) v1 = 1;
+                while ((i64)v1 * (v1 - 1) / 2 > e) --v1;
+                while ((i64)(v1 + 1) * v1 / 2 <= e) ++v1;
+                x = (int)(e - (i64)v1 * (v1 - 1) / 2);
+            }
 
-            for (int off = lane; off - lane < row_len; off += 32) {
-                const bool valid = off < row_len;
-                const int x = valid ? v0 + off : 0;
+            for (int off = lane; off - lane < seg; off += 32, lane_advance(v1, x)) {
+                const bool valid = off < seg;
                 const u64 ci = idx + (u64)off;
                 bool keep = false;
-                u32 key1 = up1;
+                u32 key1 = up2;
+                const KT* row1 = Kf + v1 * pitch;
                 if (valid) {
 #pragma unroll
-                    for (int j = 1; j < M; ++j) key1 = min(key1, (u32)Kf[v[j] * pitch + x]);
+                    for (int j = 2; j < M; ++j) key1 = min(key1, (u32)Kf[v[j] * pitch + v1]);
+                    key1 = min(key1, (u32)row1[x]);
+#pragma unroll
+                    for (int j = 2; j < M; ++j) key1 = min(key1, (u32)Kf[v[j] * pitch + x]);
                     if (key1 >= thr1) {
                         bool clr;
                         if (p.clear.bitmap) clr = (__ldg(p.clear.bitmap + (ci >> 5)) >> (ci & 31)) & 1u;
@@ -194,12 +207,12 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 if (count_only) continue;
 
                 // ---- a7, fast path: cofacet vertices n-1, n-2, ... against the row's window
-                const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | lowbase | (u64)(u32)x) : csentinel;
+                const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | slab_low | ((u64)(u32)v1 << vbits) | (u64)(u32)x) : csentinel;
                 int fv = -1;
                 const KT* rowx = Kf + x * pitch;
                 if (keep) { // each lane on its own, up to kfast vertices (the common case ends after one or two)
                     for (int k = 0; k < kfast; ++k) {
-                        if (min(uw[k], (u32)rowx[n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
+                        if (min(min(uw[k], (u32)row1[n - 1 - k]), (u32)rowx[n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
                     }
                 }
                 // the lanes still scanning are finished by the whole warp, one after the other: 32 cofacet
@@ -209,15 +222,16 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                     const int src = __ffs(open) - 1;
                     open &= open - 1;
                     const int xs = __shfl_sync(RIPS_FULL_MASK, x, src);
+                    const int v1s = __shfl_sync(RIPS_FULL_MASK, v1, src);
                     const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
                     int res = -1;
                     for (int base = n - 1 - kfast; base >= 0; base -= 32) {
                         const int vv = base - lane;
                         bool ok = false;
                         if (vv >= 0) {
-                            u32 m = (u32)Kf[xs * pitch + vv];
+                            u32 m = min((u32)Kf[xs * pitch + vv], (u32)Kf[v1s * pitch + vv]);
 #pragma unroll
-                            for (int j = 1; j < M; ++j) m = min(m, (u32)Kf[v[j] * pitch + vv]);
+                            for (int j = 2; j < M; ++j) m = min(m, (u32)Kf[v[j] * pitch + vv]);
                             ok = m >= ks;
                         }
                         const u32 b = __ballot_sync(RIPS_FULL_MASK, ok);
@@ -226,6 +240,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                     if (lane == src) fv = res;
                 }
                 const bool found = keep && fv >= 0;
+                const int vtop = (M > 2) ? v[M - 1] : v1;
                 const bool regular = found && fv > vtop;
                 u64 prec = psentinel;
                 if (regular) {
@@ -239,8 +254,9 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 if (found && !regular) {
                     int sv[M];
                     sv[0] = x;
+                    sv[1] = v1;
 #pragma unroll
-                    for (int j = 1; j < M; ++j) sv[j] = v[j];
+                    for (int j = 2; j < M; ++j) sv[j] = v[j];
                     int fseg = 0;
 #pragma unroll
                     for (int j = 0; j < M; ++j) fseg += (sv[j] < fv) ? 1 : 0;
@@ -293,15 +309,12 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                     }
                 }
             }
-            idx += (u64)row_len;
-            rem -= row_len;
-            // ---- next row (colex successor of (v[M-1..1]))
-            v0 = 0;
-            v[1] += 1;
-            if (M > 2) {
-                if (v[1] == v[M > 2 ? 2 : 1]) {
-                    new_upper = true;
-                    v[1] = 1;
+            idx += (u64)seg;
+            rem -= seg;
+            e0 += seg;
+            if (e0 >= slab_len) { // next slab (colex successor of (v[M-1..2]))
+                e0 = 0;
+                if (M > 2) {
 #pragma unroll
                     for (int j = 2; j < M; ++j) {
                         v[j] += 1;
