@@ -299,7 +299,7 @@ def run_b200(args):
     ev0.record()
     for _ in range(args.steps):
         hot_step()
-        for d in range(1, D + 1):   # events recorded by the library on the same stream; already complete
+        for d in range(1, D + 1):   # the library's own CUDA events of this step, read once the step is enqueued
             t = g.timings(d)
             for k in KERNELS:
                 per_kernel[k] += t[k]
@@ -336,6 +336,13 @@ def run_b200(args):
             tj = json.load(f)
         key = f"cfg{args.config}:{top['kernel'].split(' ')[0]}:{'a9' if 'a9' in top['kernel'] else 'a6' if 'a6' in top['kernel'] else ''}"
         roofline["traffic"] = tj.get(key)
+        inst = tj.get(key + ":inst")
+        if inst and top["ms_per_launch"] > 0:
+            # the fused kernel is bound by instruction issue, not by HBM: 148 SMs x 4 schedulers x 1.965 GHz
+            peak_inst = 148 * 4 * 1.965e9
+            roofline["issue"] = {"warp_inst_per_launch": inst, "achieved_ginst_s": inst / (top["ms_per_launch"] * 1e-3) / 1e9,
+                                 "peak_ginst_s": peak_inst / 1e9, "frac": inst / (top["ms_per_launch"] * 1e-3) / peak_inst,
+                                 "note": "ncu smsp__inst_executed.sum / live duration; what actually binds this kernel"}
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     e2e_ms, d2h_bytes, parts = [], 0, None
