@@ -56,7 +56,7 @@ struct FusedHist {
     int shift[4], bits[4];
 };
 // Counters written by the fused kernel (u64 each)
-enum { S1C_KEPT = 0, S1C_OVER = 1, S1C_CLEARED = 2, S1C_REGULAR = 3, S1C_IRREGULAR = 4, S1C_NONAPP = 5 };
+enum { S1C_KEPT = 0, S1C_OVER = 1, S1C_CLEARED = 2, S1C_REGULAR = 3, S1C_IRREGULAR = 4, S1C_NONAPP = 5, S1C_STAGE_OVERFLOW = 6 };
 
 struct Stage1Params {
     const void* Kf;   // full key matrix (u16 or u32, see launch_stage1's kf_u16), row pitch `pitch` entries
@@ -66,6 +66,7 @@ struct Stage1Params {
     u64 total;        // C(n, d+1)
     i64 tiles;        // warp chunks
     int chunk;        // candidates per warp chunk (stage1_chunk)
+    int stage_cap;    // compact mode: records a warp can stage per chunk (stage1_stage_cap)
     u32 thr_key;      // keep iff key >= thr_key
     u32 sentinel_key; // key field of the column sentinel (= number of distinct keys, larger than every key)
     int vbits, lowbits;
@@ -86,7 +87,8 @@ struct Stage1Params {
     FusedHist fh_cols;   // digit histogram of the filtration sort (over every slot written to cols_out)
     FusedHist fh_pairs;  // digit histogram of the partition of pairs_out by v
 };
-int stage1_chunk(u64 total, int compact);
+int stage1_chunk(u64 total, int compact, double est_survival, int retry);
+int stage1_stage_cap();
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
 // bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask
 cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st);

@@ -346,9 +346,10 @@ int run_stage1(rips_ctx* c, int d)
     // any), so every candidate keeps its slot; with one, estimate the surviving share from the share
     // q of admissible edges (q^(edges of the simplex)) and compact when most are dropped
     const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
-    s.compact = (c->thr_key != 0 && std::pow(q, (double)(s.M * (s.M - 1) / 2)) < 0.5) ? 1 : 0;
-    const int chunk = stage1_chunk(s.total, s.compact);
-    const i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
+    const double est_survival = std::pow(q, (double)(s.M * (s.M - 1) / 2));
+    s.compact = (c->thr_key != 0 && est_survival < 0.5) ? 1 : 0;
+    int chunk = stage1_chunk(s.total, s.compact, est_survival, 0);
+    i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
     Stage1Params p;
     p.Kf = c->d_Kf;
     p.pitch = c->kf_pitch;
@@ -357,6 +358,7 @@ int run_stage1(rips_ctx* c, int d)
     p.total = s.total;
     p.tiles = tiles;
     p.chunk = chunk;
+    p.stage_cap = stage1_stage_cap();
     p.thr_key = c->thr_key;
     p.sentinel_key = c->n_distinct;
     p.vbits = c->vbits;
@@ -467,9 +469,18 @@ int run_stage1(rips_ctx* c, int d)
             CU(cudaStreamSynchronize(c->stream));
         }
         const u64 ni = c->h_counters[S1C_IRREGULAR], nn = c->h_counters[S1C_NONAPP];
-        if (ni <= irr_cap && nn <= non_cap) break;
+        const bool stage_overflow = c->h_counters[S1C_STAGE_OVERFLOW] != 0;
+        if (ni <= irr_cap && nn <= non_cap && !stage_overflow) break;
         if (sorted_early) { CU(cudaStreamSynchronize(c->stream)); sorted_early = false; }
-        if (attempt >= 1) { g_last_error = "rips_stage1: list capacities still too small on the second attempt"; return RIPS_ECUDA; }
+        if (stage_overflow) { // a chunk kept more than a warp can stage: again with chunks no longer than the staging
+            chunk = stage1_chunk(s.total, s.compact, est_survival, 1);
+            tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
+            p.chunk = chunk;
+            p.tiles = tiles;
+            RC(ensure(c, s.s1_status, (size_t)tiles * 8));
+            p.status = (u64*)s.s1_status.p;
+        }
+        if (attempt >= 2) { g_last_error = "rips_stage1: list capacities still too small on the second attempt"; return RIPS_ECUDA; }
         irr_cap = std::max(irr_cap, ni); // rare: more irregular pairs / non-apparent columns than provisioned; run again
         non_cap = std::max(non_cap, nn);
     }

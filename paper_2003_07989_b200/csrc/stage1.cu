@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     u64* stage_cols = nullptr;
     u64* stage_pairs = nullptr;
     if (compact && !count_only) {
-        stage_cols = reinterpret_cast<u64*>(smem1 + off_b) + (size_t)warp * (2 * p.chunk);
-        stage_pairs = stage_cols + p.chunk;
+        stage_cols = reinterpret_cast<u64*>(smem1 + off_b) + (size_t)warp * (2 * p.stage_cap);
+        stage_pairs = stage_cols + p.stage_cap;
     }
     BlockHists H;
     H.cols = s_hist_cols;
@@ -127,14 +127,32 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     const int kfast = p.fast_visits < kwin ? p.fast_visits : kwin; // vertices n-1 .. n-kfast: per-lane scan of the row's window
     u32* const uw = s_uwin[warp];
 
+    // Compact mode: the unit of the look-back chain is a ROUND of the block (one chunk per warp), so that the
+    // chain has S1_WARPS times fewer links than chunks (with most candidates dropped the chunks are cheap, and a
+    // chain of one link per chunk was what bounded the kernel).  Slot mode needs no chain: warps take chunks alone.
+    const bool block_rounds = compact && !count_only;
+    __shared__ u32 s_round;
+    __shared__ u32 s_wc[S1_WARPS];
+    __shared__ u64 s_excl;
     for (;;) {
-        u32 chunk = 0;
-        if (lane == 0) chunk = atomicAdd(p.ticket, 1u);
-        chunk = __shfl_sync(RIPS_FULL_MASK, chunk, 0);
-        if ((i64)chunk >= p.tiles) break;
+        u32 chunk = 0, round = 0;
+        bool active = true;
+        if (block_rounds) {
+            __syncthreads(); // the previous round's shared words are no longer read
+            if (tid == 0) s_round = atomicAdd(p.ticket, 1u);
+            __syncthreads();
+            round = s_round;
+            if ((i64)round * S1_WARPS >= p.tiles) break;
+            chunk = round * S1_WARPS + warp;
+            active = (i64)chunk < p.tiles;
+        } else {
+            if (lane == 0) chunk = atomicAdd(p.ticket, 1u);
+            chunk = __shfl_sync(RIPS_FULL_MASK, chunk, 0);
+            if ((i64)chunk >= p.tiles) break;
+        }
 
-        u64 idx = (u64)chunk * (u64)p.chunk;
-        int rem = (p.total - idx) < (u64)p.chunk ? (int)(p.total - idx) : p.chunk;
+        u64 idx = active ? (u64)chunk * (u64)p.chunk : 0;
+        int rem = !active ? 0 : (p.total - idx) < (u64)p.chunk ? (int)(p.total - idx) : p.chunk;
         int v[M];
         decode_simplex_fast<M>(p.bt, idx, n, v); // warp-uniform
         u32 wcount = 0;
@@ -204,7 +222,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 const u32 bal = __ballot_sync(RIPS_FULL_MASK, keep);
                 const u32 slot = wcount + __popc(bal & lt_mask);
                 wcount += __popc(bal);
-                if (count_only) continue;
+                if (count_only || (compact && bal == 0)) continue; // compact mode writes nothing for an all-dropped warp step
 
                 // ---- a7, fast path: cofacet vertices n-1, n-2, ... against the row's window
                 const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | slab_low | ((u64)(u32)v1 << vbits) | (u64)(u32)x) : csentinel;
@@ -285,8 +303,11 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 // ---- stores
                 if (compact) {
                     if (keep) {
-                        stage_cols[slot] = rec;
-                        stage_pairs[slot] = prec;
+                        if (slot < (u32)p.stage_cap) {
+                            stage_cols[slot] = rec;
+                            stage_pairs[slot] = prec;
+                        } else // more survivors than provisioned for this chunk: the host repeats the launch with smaller chunks
+                            atomicOr((unsigned long long*)(p.counters + S1C_STAGE_OVERFLOW), 1ull);
                     }
                 } else if (valid) {
                     __stcs(p.cols_out + ci, rec);
@@ -328,10 +349,19 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
         n_kept += wcount;
         if (count_only) continue;
         if (compact) {
-            // ---- ordered compaction: warp-level look-back over the chunks
-            const u64 excl = lookback_exclusive(p.status, (i64)chunk, (u64)wcount);
-            __syncwarp();
-            for (u32 i = lane; i < wcount; i += 32) {
+            // ---- ordered compaction: look-back over the block's rounds, then every warp writes its staged records
+            if (lane == 0) s_wc[warp] = wcount;
+            __syncthreads();
+            if (warp == 0) {
+                u32 c = lane < S1_WARPS ? s_wc[lane] : 0u;
+                const u64 total_round = (u64)__reduce_add_sync(RIPS_FULL_MASK, c);
+                const u64 e = lookback_exclusive(p.status, (i64)round, total_round);
+                if (lane == 0) s_excl = e;
+            }
+            __syncthreads();
+            u64 excl = s_excl;
+            for (int w = 0; w < warp; ++w) excl += s_wc[w];
+            for (u32 i = lane; i < wcount && i < (u32)p.stage_cap; i += 32) {
                 __stcs(p.cols_out + excl + i, stage_cols[i]);
                 __stcs(p.pairs_out + excl + i, stage_pairs[i]);
             }
@@ -376,7 +406,7 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
     static const bool kf_global = getenv("RIPS_KF_GLOBAL") != nullptr; // tuning: never stage Kf in shared memory
     const int k_in = (!kf_global && !p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
     const size_t smem = (k_in ? kf_bytes : 0) +
-                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.chunk * 8 : 0);
+                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.stage_cap * 8 : 0);
     auto kern = k_in ? enumerate_apparent_kernel<M, KT, true> : enumerate_apparent_kernel<M, KT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) return e;
@@ -395,14 +425,26 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 } // namespace
 
 // Candidates per warp chunk: S1_CHUNK when there is plenty of work, less (a multiple of 32) when the
-// index space is small, so that every SM still gets warps to run.
-int stage1_chunk(u64 total, int compact)
+// index space is small, so that every SM still gets warps to run.  Compact mode stages the survivors of
+// a chunk in shared memory (S1_STAGE_CAP records per warp) and wants long chunks, because every round of
+// chunks is a link of the look-back chain: the chunk is sized so that the expected survivors
+// (est_survival x chunk) fill half the staging; a chunk that overflows is reported and the launch repeated
+// with chunk = S1_STAGE_CAP (retry != 0).
+int stage1_stage_cap() { return 256; }
+int stage1_chunk(u64 total, int compact, double est_survival, int retry)
 {
     u64 c = (total / (148ull * 64) + 31) / 32 * 32;
     if (c < 32) c = 32;
-    if (c > (u64)S1_CHUNK) c = S1_CHUNK;
-    if (compact && c > 256) c = 256; // two staged records per candidate and warp must fit shared memory
-    return (int)c;
+    if (!compact) return (int)(c > (u64)S1_CHUNK ? (u64)S1_CHUNK : c);
+    const u64 cap = (u64)stage1_stage_cap();
+    u64 want = cap;
+    if (!retry) {
+        const double e = est_survival > 1e-3 ? est_survival : 1e-3;
+        want = (u64)(0.5 * (double)cap / e) / 32 * 32;
+        if (want < cap) want = cap;
+        if (want > 4096) want = 4096;
+    }
+    return (int)(c < want ? c : want);
 }
 
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st)

@@ -177,3 +177,40 @@ def test_second_workload_dim1_random_permutation_matrix(R):
         nd, nc = g.nonapparent(1)
         m = (nc >= lo) & (nc < hi)
         assert np.array_equal(torch.sort(nc[m])[0].cpu().numpy().astype(np.uint64), np.sort(s2["non_cidx"]))
+
+
+def test_compact_mode_with_dense_runs(R):
+    """Thresholded input whose survivors come in long dense runs of the index space (two tight clusters far
+    apart, threshold between the two scales): the estimate of the surviving share is low, so compact mode picks
+    long chunks, the chunks inside a cluster overflow the staging, and the launch is repeated with short ones.
+    The result must not depend on any of that."""
+    import torch
+    n = 400
+    rng = np.random.default_rng(5)
+    pts = rng.random((n, 3), dtype=np.float32) * 0.05
+    pts[n // 2:] += 10.0
+    low = inputs.euclidean_lower(pts)
+    thr = 1.0
+    z = oracle.dim0(low, n, thr)
+    fd1, fc1, _ = oracle.stage1(low, n, 1, thr, z["t"])
+    s21 = oracle.stage2(low, n, 1, fd1, fc1)
+    red = oracle.reduce_columns(low, n, 1, thr, s21["non_cidx"], s21["app_t"], s21["app_s"])
+    cleared2 = np.sort(np.concatenate([s21["app_t"], red["t"]]))
+    od, oc, counts = oracle.stage1(low, n, 2, thr, cleared2)
+    s2 = oracle.stage2(low, n, 2, od, oc)
+    with R.Rips(low, n, 2, thr) as g:
+        g.dim0()
+        g.stage1(1); g.stage2(1); g.reduce(1)
+        g.stage1(2); g.stage2(2)
+        st = g.stats(2)
+        assert st["n_slots"] == st["n_columns"]          # compact mode
+        assert (st["n_columns"], st["n_removed_by_diameter"], st["n_cleared"]) == \
+               (counts["kept"], counts["removed_by_diameter"], counts["cleared"])
+        fd, fc = g.filtration(2)
+        assert np.array_equal(fc.cpu().numpy().astype(np.uint64), oc)
+        assert np.array_equal(fd.cpu().numpy().view(np.uint32), od.view(np.uint32))
+        at, as_ = g.apparent_pairs(2)
+        assert np.array_equal(at.cpu().numpy().astype(np.uint64), s2["app_t"])
+        assert np.array_equal(as_.cpu().numpy().astype(np.uint64), s2["app_s"])
+        nd, nc = g.nonapparent(2)
+        assert np.array_equal(nc.cpu().numpy().astype(np.uint64), s2["non_cidx"])
