@@ -13,6 +13,13 @@
  *            the pairs (t, s) sorted by t with a binary-search lookup, the
  *            non-apparent columns kept in coboundary order.
  *
+ * How the work is split between the two entry points: the apparent test of a
+ * column does not depend on the order of the columns (Corollary 8), so it runs
+ * inside the kernel of rips_stage1 that enumerates the candidates, where the column's vertices and
+ * diameter are in registers; rips_stage1 then sorts the columns, and rips_stage2 puts the pairs and the
+ * non-apparent columns that kernel produced into their sorted order.  The arrays each call exposes are
+ * the paper's, whatever the split.
+ *
  * Dimension 0 and the reduction of the non-apparent columns (Algorithm 2,
  * PAPER.md:182-200) complete the barcodes; they are not the hot path and are timed separately
  * (rips_timings).  Every step of stage 1 and stage 2 runs in hand-written CUDA kernels for
@@ -48,7 +55,7 @@ enum {
                             NaN threshold, d out of range, stage called before its inputs exist */
     RIPS_EOVERFLOW = -2, /* C(n, dim_max+3) >= 2^63, n >= 65536, or (rank bits + index bits) > 64 so a
                             column does not fit the packed 64-bit record */
-    RIPS_ENOMEM = -3,    /* device or host allocation failed / caller's workspace too small */
+    RIPS_ENOMEM = -3,    /* device or host allocation failed */
     RIPS_ECUDA = -4      /* CUDA runtime error; text via rips_last_error */
 };
 
@@ -58,7 +65,7 @@ typedef struct {
     int64_t n_removed_by_diameter; /* diameter > threshold */
     int64_t n_cleared;             /* diameter <= threshold and cleared */
     int64_t n_columns;             /* kept = length of the filtration array */
-    int64_t n_apparent;            /* apparent pairs found by stage 2 */
+    int64_t n_apparent;            /* apparent pairs (Definition 5) among the columns */
     int64_t n_nonapparent;         /* columns left for the reduction */
     int64_t n_reduced_pivots;      /* pairs found by the reduction */
     int64_t n_essential;           /* columns that reduce to zero */
@@ -93,7 +100,7 @@ typedef struct {
     float reduce_xfer_ms;    /* NOT hot path: D2H/H2D copies around the host reduction */
 } rips_timings_t;
 
-/* Exact upper bound, in bytes, of the device memory rips_compute needs for (n, dim_max) with no
+/* Estimate (an upper bound up to allocator rounding), in bytes, of the device memory rips_compute holds for (n, dim_max) with no
  * threshold (a threshold only lowers it).  RIPS_EOVERFLOW if the sizes do not fit. */
 int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes);
 
@@ -118,7 +125,7 @@ int rips_dim0(rips_ctx* ctx);
 int rips_stage1(rips_ctx* ctx, int d);
 int rips_stage2(rips_ctx* ctx, int d);
 /* Reduction of the non-apparent columns of dimension d (after rips_stage2(d)); completes the pivots
- * of dimension d.  Not the hot path: runs Algorithm 2 serially on the host, timed separately. */
+ * of dimension d.  Not the hot path, timed separately. */
 int rips_reduce(rips_ctx* ctx, int d);
 /* Alternative to rips_reduce(d) for a reduction done elsewhere (the paper's own split runs it on the
  * host): installs `count` pivots (t_host[i], s_host[i]), HOST arrays ascending by t, as the

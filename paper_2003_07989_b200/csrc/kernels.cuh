@@ -1,13 +1,13 @@
-// kernels.cuh -- host-side launchers of the hot-path kernels (definitions in stage1.cu, stage2.cu,
-// dim0.cu, init.cu).  Packed records used throughout the device path:
+// kernels.cuh -- host-side launchers of the kernels (definitions in stage1.cu, stage2.cu, dim0.cu,
+// init.cu, reduce.cu).  Packed records used throughout the device path:
 //
 //   column record   (key << lowbits) | verts   key = descending dense rank of the diameter (0 = largest
 //                                               distance); verts = the simplex's vertices, v[j] at bit
 //                                               j*vbits, vbits = bits of n-1, lowbits = (d+1)*vbits.
 //                                               The vertex word orders simplices exactly like cidx does
 //                                               (colex order = lexicographic on the decreasing vertex
-//                                               tuple, Remark 2), and spares stage 2 and
-//                                               the unpack kernels the inverse of Eq. 2.
+//                                               tuple, Remark 2), and spares every consumer
+//                                               the inverse of Eq. 2.
 //   regular pair    (v << tbits) | cidx(t)     v = the cofacet vertex, above every vertex of s (apparent.cuh)
 //   irregular pair  (cidx(t) << 3) | j         j = position of the added vertex v inside t
 //                                               (number of vertices of s below v); s = t minus that vertex
@@ -52,7 +52,7 @@ struct ClearSet {
 // digits of a radix sort whose histogram a producer kernel accumulates while it writes the records
 struct FusedHist {
     u64* hist;        // [npasses][256] raw counts, zeroed by the caller; NULL = not fused
-    int npasses;      // <= 4
+    int npasses;      // <= 3 for the filtration sort, <= 2 for the pair partition (S1_MAX_FUSED, S1_MAX_FUSED_P)
     int shift[4], bits[4];
 };
 // Counters written by the fused kernel (u64 each)

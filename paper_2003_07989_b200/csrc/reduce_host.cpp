@@ -6,7 +6,6 @@
 // PAPER.md:77-79), i.e. simply the largest packed entry.
 #include "reduce_host.h"
 
-#include <chrono>
 #include <functional>
 #include <cstdio>
 #include <cstdlib>
@@ -214,7 +213,6 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
         }
         ++n_slow;
         const int64_t adds0 = out.additions;
-        const auto tc0 = std::chrono::steady_clock::now();
         store.clear();
         Heap h(std::less<uint64_t>(), std::move(store));
         cx.push_coboundary(h, cidx_s);
@@ -251,12 +249,6 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
             h.push(piv); // the column of s2 contains t as well: the two cancel
             cx.push_coboundary(h, s2);
             ++out.additions;
-        }
-        {
-            double ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - tc0).count();
-            if (getenv("RIPS_DEBUG") && ms > 20.0)
-                fprintf(stderr, "  slow column %lld: %.1f ms, %lld additions, heap %zu, pre %llx\n", (long long)j, ms,
-                        (long long)(out.additions - adds0), h.size(), (unsigned long long)(in.pre ? in.pre[j] : 0));
         }
     }
     if (getenv("RIPS_DEBUG"))
