@@ -34,8 +34,9 @@
  *   - Pointers named *_dev are device pointers, *_host host pointers.  Every output array is
  *     owned by the context and stays valid until the next call that recomputes it (rips_compute,
  *     rips_stage1/2 for the same d) or rips_free.  The input matrix is copied by rips_init.
- *   - All work is enqueued on the stream given to rips_init; calls that return host-visible
- *     counts synchronise that stream.
+ *   - All work is enqueued on the stream given to rips_init (rips_stage2 also uses internal streams,
+ *     joined back into that stream before it returns); calls that return host-visible counts
+ *     synchronise that stream.
  *   - Not thread-safe per context; distinct contexts are independent.
  */
 #ifndef RIPS_H
