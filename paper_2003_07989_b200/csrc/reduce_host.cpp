@@ -10,7 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 
-#include <queue>
+#include <algorithm>
 #include <unordered_map>
 
 namespace {
@@ -109,6 +109,69 @@ struct Ctx {
     }
 };
 
+// Working column of the reduction: a multiset of packed entries (key << tbits | cidx(t)) with "largest
+// first" access.  The pivots of a column come out in (almost always) decreasing order -- whatever an
+// addition brings in lies later in the filtration than the pivot it cancels, except for the unreduced
+// column of an earlier non-apparent owner -- so instead of one big heap the entries are kept in one
+// bucket per key: only the bucket of the current key is a heap (small, cache-resident), the others are
+// plain vectors that are heapified when the sweep reaches them.
+class KeyedColumn {
+public:
+    KeyedColumn(uint32_t n_keys, int tbits) : tbits_(tbits), buckets_(n_keys + 1) {}
+    void clear()
+    {
+        for (uint32_t k : touched_) buckets_[k].clear();
+        touched_.clear();
+        cur_ = -1;
+        size_ = 0;
+    }
+    void push(uint64_t e)
+    {
+        const int64_t k = (int64_t)(e >> tbits_);
+        std::vector<uint64_t>& b = buckets_[(size_t)k];
+        if (b.empty()) touched_.push_back((uint32_t)k);
+        b.push_back(e);
+        ++size_;
+        if (k == cur_) std::push_heap(b.begin(), b.end());
+        else if (k > cur_) cur_ = -1; // an entry above the sweep position: find the top again at the next access
+        if (k > max_key_) max_key_ = k;
+    }
+    bool empty() { return !settle(); }
+    uint64_t top() { settle(); return buckets_[(size_t)cur_].front(); }
+    void pop()
+    {
+        settle();
+        std::vector<uint64_t>& b = buckets_[(size_t)cur_];
+        std::pop_heap(b.begin(), b.end());
+        b.pop_back();
+        --size_;
+    }
+    size_t size() const { return size_; }
+
+private:
+    // make cur_ the largest key with a non-empty bucket, its bucket a heap; false if the column is empty
+    bool settle()
+    {
+        if (cur_ >= 0 && !buckets_[(size_t)cur_].empty()) return true;
+        if (size_ == 0) return false;
+        int64_t k = (cur_ >= 0) ? cur_ : max_key_;
+        while (k >= 0 && buckets_[(size_t)k].empty()) --k;
+        if (k < 0) { // entries only above the old position (cannot happen when cur_ < 0)
+            k = max_key_;
+            while (buckets_[(size_t)k].empty()) --k;
+        }
+        if (cur_ < 0) max_key_ = k;
+        cur_ = k;
+        std::make_heap(buckets_[(size_t)k].begin(), buckets_[(size_t)k].end());
+        return true;
+    }
+    int tbits_;
+    std::vector<std::vector<uint64_t>> buckets_;
+    std::vector<uint32_t> touched_;
+    int64_t cur_ = -1, max_key_ = 0;
+    size_t size_ = 0;
+};
+
 template <class Heap>
 bool pop_pivot(Heap& h, uint64_t* piv)
 {
@@ -127,15 +190,15 @@ bool pop_pivot(Heap& h, uint64_t* piv)
 // Oblivious column reduction (Algorithm 2) of the columns in coboundary order.  A
 // column the device has already reduced against the apparent columns (in.pre) and whose pivot no
 // earlier column owns is final at once; the others -- the conflicts between non-apparent columns, a
-// fraction of a per cent of the columns at the paper-shaped workloads -- are reduced here, a heap as
-// the working column, adding D_{lookup[low]} whether the pivot's owner is an apparent column or one
+// fraction of a per cent of the columns at the paper-shaped workloads -- are reduced here (KeyedColumn as
+// the working column), adding D_{lookup[low]} whether the pivot's owner is an apparent column or one
 // reduced earlier (Lemma 3: same result as adding R_i).
 void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
 {
     Ctx cx(in);
     const uint64_t cmask = (in.cbits >= 64) ? ~0ull : ((1ull << in.cbits) - 1ull);
     const uint64_t tmask = (1ull << in.tbits) - 1ull;
-    typedef std::priority_queue<uint64_t, std::vector<uint64_t>> Heap;
+    typedef KeyedColumn Heap;
     std::unordered_map<uint64_t, uint64_t> owner; // second layer: t -> cidx(s) of the column that owns the pivot
     owner.reserve((size_t)in.ncols * 2 + 16);
     auto finalize = [&](int64_t j, uint64_t piv, uint64_t cidx_s, uint32_t key_s) {
@@ -156,7 +219,7 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
     int64_t n_vmode = 0;
     std::function<const std::vector<uint64_t>&(uint64_t, uint64_t*)> reduce_v =
         [&](uint64_t cidx_s, uint64_t* piv_out) -> const std::vector<uint64_t>& {
-        Heap h;
+        Heap h(in.n_keys, in.tbits);
         std::unordered_map<uint64_t, int> par; // column -> parity in V
         auto add_col = [&](uint64_t c) { cx.push_coboundary(h, c); par[c] ^= 1; };
         add_col(cidx_s);
@@ -195,7 +258,7 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
     };
     const int64_t oblivious_budget = 256; // additions before a column is restarted with the V technique
     int64_t n_fast = 0, n_slow = 0, n_def = 0, n_own_adds = 0;
-    std::vector<uint64_t> store;
+    Heap h(in.n_keys, in.tbits);
     for (int64_t j = 0; j < in.ncols; ++j) {
         const uint64_t cidx_s = in.cols[j] & cmask;
         const uint32_t key_s = (uint32_t)(in.cols[j] >> in.cbits);
@@ -213,8 +276,7 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
         }
         ++n_slow;
         const int64_t adds0 = out.additions;
-        store.clear();
-        Heap h(std::less<uint64_t>(), std::move(store));
+        h.clear();
         cx.push_coboundary(h, cidx_s);
         for (;;) {
             uint64_t piv;

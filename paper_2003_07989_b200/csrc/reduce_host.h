@@ -11,6 +11,7 @@ struct HostReduceIn {
     const uint64_t* binom;    // host binomial table, k-major, stride n+1
     int bstride;
     uint32_t thr_key;         // cofacets with key < thr_key are above the threshold
+    uint32_t n_keys;          // number of distinct keys (keys are 0 .. n_keys-1)
     const uint64_t* cols;     // packed column records of the non-apparent columns, coboundary order
     int64_t ncols;
     int cbits;

@@ -629,6 +629,7 @@ int run_reduce(rips_ctx* c, int d)
         in.binom = c->h_binom.data();
         in.bstride = (int)(c->n + 1);
         in.thr_key = c->thr_key;
+        in.n_keys = c->n_distinct;
         in.cols = h_non.data();
         in.ncols = s.n_non;
         in.cbits = s.cbits;
