@@ -167,3 +167,20 @@ def test_scale_row_entry_points(R):
         g.stage1(3); g.stage2(3)
         at2, _ = g.apparent_pairs(3)
         assert bool((at2 == at).all())
+
+
+def test_dim_max_4(R):
+    """The widest instantiations (columns of 5 vertices, cofacets of 6), every array against the oracle."""
+    w = inputs.config(2, 13)
+    check_against_oracle(R, w.dist, w.n, 4, inf, "dim_max 4")
+    w = inputs.config(1, 12)
+    thr = float(np.float32(np.quantile(w.dist, 0.6)))
+    check_against_oracle(R, w.dist, w.n, 4, thr, "dim_max 4 with a threshold")
+
+
+def test_more_than_256_vertices(R):
+    """n > 256: vertex fields of 9 bits and a pair partition of two radix passes."""
+    w = inputs.config(1, 300)
+    check_against_oracle(R, w.dist, w.n, 1, inf, "n = 300, dimension 1")
+    thr = float(np.float32(np.quantile(w.dist, 0.05)))
+    check_against_oracle(R, w.dist, w.n, 2, thr, "n = 300, dimension 2, 5 % of the edges")
