@@ -30,9 +30,15 @@ __device__ __forceinline__ u32 find_root(volatile u32* parent, u32 x)
     return r;
 }
 
+// SM: the union-find arrays (parent, largest vertex per root: 8 bytes per vertex) live in shared memory
+// (n <= 25000); else in the global scratch the caller passed.  The merges are serial, so their latency is
+// the kernel's run time.
+template <bool SM>
 __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict__ rec, i64 E, int n, u32 thr_inv,
                                                           u32* parent_maxv, Dim0Out out)
 {
+    extern __shared__ u32 s_uf[];
+    if (SM) parent_maxv = s_uf;
     __shared__ u32 s_list[D0_THREADS];
     __shared__ u32 s_wcount[D0_THREADS / 32];
     __shared__ i64 s_start;
@@ -103,6 +109,12 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
 cudaError_t launch_dim0(const u64* rec_sorted, i64 E, int n, u32 thr_bits_inv, u32* parent_maxv, Dim0Out out,
                         cudaStream_t st)
 {
-    dim0_kernel<<<1, D0_THREADS, 0, st>>>(rec_sorted, E, n, thr_bits_inv, parent_maxv, out);
+    const size_t bytes = (size_t)n * 8;
+    if (bytes <= 200 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(dim0_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return e;
+        dim0_kernel<true><<<1, D0_THREADS, bytes, st>>>(rec_sorted, E, n, thr_bits_inv, parent_maxv, out);
+    } else
+        dim0_kernel<false><<<1, D0_THREADS, 0, st>>>(rec_sorted, E, n, thr_bits_inv, parent_maxv, out);
     return cudaGetLastError();
 }
