@@ -224,6 +224,16 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
             i64 t = tile - 1;
             bool done = false;
             while (!done) {
+                // wait (one word, with a back-off) until the nearest tile not yet summed is published; the
+                // tiles before it are older and almost always published already, so they are read as a batch
+                u64 s0 = ld_volatile_u64(status + t * nbins + tid);
+                while ((s0 >> 62) == 0) {
+                    __nanosleep(40);
+                    s0 = ld_volatile_u64(status + t * nbins + tid);
+                }
+                excl += s0 & LB_VALUE_MASK;
+                --t;
+                if ((s0 >> 62) == 2 || t < 0) break;
                 u64 sv[SORT_LB_BATCH];
 #pragma unroll
                 for (int b = 0; b < SORT_LB_BATCH; ++b)
@@ -232,10 +242,10 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
                 for (int b = 0; b < SORT_LB_BATCH; ++b) {
                     if (!done) {
                         const u64 flag = sv[b] >> 62;
-                        if (flag == 0) break; // not published yet: poll again from this tile
+                        if (flag == 0) break; // not published yet: wait for this tile
                         excl += sv[b] & LB_VALUE_MASK;
                         --t;
-                        if (flag == 2) done = true;
+                        if (flag == 2 || t < 0) done = true;
                     }
                 }
             }
