@@ -121,7 +121,8 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     for (int i = tid; i < S1_MAX_FUSED_P * 256; i += S1_THREADS) (&s_hist_pairs[0][0])[i] = 0;
     __syncthreads();
 
-    u32 n_over = 0, n_clr = 0, n_reg = 0;
+    u32 n_clr = 0, n_reg = 0;
+    u64 n_over = 0;
     u64 n_kept = 0;
     const int kwin = n < 32 ? n : 32;
     const int kfast = p.fast_visits < kwin ? p.fast_visits : kwin; // vertices n-1 .. n-kfast: per-lane scan of the row's window
@@ -185,20 +186,8 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 uw[lane] = u;
                 __syncwarp();
             }
-            // ---- this lane's first pair (v1, x) of the segment: e = C(v1, 2) + x
-            int v1, x;
-            {
-                const i64 e = e0 + lane;
-                v1 = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)e)) * 0.5f);
-                if (v1 < 1) v1 = 1;
-                while ((i64)v1 * (v1 - 1) / 2 > e) --v1;
-                while ((i64)(v1 + 1) * v1 / 2 <= e) ++v1;
-                x = (int)(e - (i64)v1 * (v1 - 1) / 2);
-            }
-
-            for (int off = lane; off - lane < seg; off += 32, lane_advance(v1, x)) {
-                const bool valid = off < seg;
-                const u64 ci = idx + (u64)off;
+            // one warp step: this lane's candidate (v[M-1..2], v1, x) with index ci
+            auto step = [&](const int v1, const int x, const bool valid, const u64 ci) {
                 bool keep = false;
                 u32 key1 = up2;
                 const KT* row1 = Kf + v1 * pitch;
@@ -222,7 +211,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                 const u32 bal = __ballot_sync(RIPS_FULL_MASK, keep);
                 const u32 slot = wcount + __popc(bal & lt_mask);
                 wcount += __popc(bal);
-                if (count_only || (compact && bal == 0)) continue; // compact mode writes nothing for an all-dropped warp step
+                if (count_only || (compact && bal == 0)) return; // compact mode writes nothing for an all-dropped warp step
 
                 // ---- a7, fast path: cofacet vertices n-1, n-2, ... against the row's window
                 const u64 rec = keep ? (((u64)(key1 - 1u) << lowbits) | slab_low | ((u64)(u32)v1 << vbits) | (u64)(u32)x) : csentinel;
@@ -329,6 +318,52 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                         if (wrote_pair && lane == __ffs(peers) - 1) atomicAdd(&H.pairs[r][dg], (u32)__popc(peers));
                     }
                 }
+            };
+
+            if (!compact) {
+                // ---- slot mode: the lanes walk the segment's pairs (v1, x) in index order, 32 at a time
+                int lv1, lx;
+                {
+                    const i64 e = e0 + lane;
+                    lv1 = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)e)) * 0.5f);
+                    if (lv1 < 1) lv1 = 1;
+                    while ((i64)lv1 * (lv1 - 1) / 2 > e) --lv1;
+                    while ((i64)(lv1 + 1) * lv1 / 2 <= e) ++lv1;
+                    lx = (int)(e - (i64)lv1 * (lv1 - 1) / 2);
+                }
+                for (int off = lane; off - lane < seg; off += 32, lane_advance(lv1, lx))
+                    step(lv1, lx, off < seg, idx + (u64)off);
+            } else {
+                // ---- compact mode (a threshold drops most candidates): row by row, v1 warp-uniform, so that a row
+                // whose upper edges already exceed the threshold is skipped as a whole -- the pruning of the index
+                // space that makes a thresholded (sparse) complex cheap: under a threshold that keeps a share q of
+                // the edges only about q of the rows are walked at all
+                int r1;
+                {
+                    r1 = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)e0)) * 0.5f);
+                    if (r1 < 1) r1 = 1;
+                    while ((i64)r1 * (r1 - 1) / 2 > e0) --r1;
+                    while ((i64)(r1 + 1) * r1 / 2 <= e0) ++r1;
+                }
+                int x0 = (int)(e0 - (i64)r1 * (r1 - 1) / 2);
+                int left = seg;
+                u64 ci0 = idx;
+                while (left > 0) {
+                    const int row_n = min(r1 - x0, left);
+                    u32 rowkey = up2;
+#pragma unroll
+                    for (int j = 2; j < M; ++j) rowkey = min(rowkey, (u32)Kf[v[j] * pitch + r1]);
+                    if (rowkey < thr1) {
+                        if (lane == 0) n_over += (u64)row_n; // every candidate of the row is above the threshold
+                    } else {
+                        for (int off = lane; off - lane < row_n; off += 32)
+                            step(r1, x0 + off, off < row_n, ci0 + (u64)off);
+                    }
+                    ci0 += (u64)row_n;
+                    left -= row_n;
+                    x0 = 0;
+                    ++r1;
+                }
             }
             idx += (u64)seg;
             rem -= seg;
@@ -370,7 +405,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     }
 
     // ---- counters and the fused histograms: once per block
-    n_over = warp_sum_u32(n_over);
+    n_over = warp_sum_u64(n_over);
     n_clr = warp_sum_u32(n_clr);
     n_reg = warp_sum_u32(n_reg);
     if (lane == 0) {
