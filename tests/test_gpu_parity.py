@@ -184,3 +184,13 @@ def test_more_than_256_vertices(R):
     check_against_oracle(R, w.dist, w.n, 1, inf, "n = 300, dimension 1")
     thr = float(np.float32(np.quantile(w.dist, 0.05)))
     check_against_oracle(R, w.dist, w.n, 2, thr, "n = 300, dimension 2, 5 % of the edges")
+
+
+def test_workspace_estimate_bounds_what_is_held(R):
+    """rips_workspace_bytes is an upper bound of rips_device_bytes after rips_compute (accessor views excluded)."""
+    for k, n in [(1, 50), (2, 60), (5, 120)]:
+        w = inputs.config(k, n)
+        thr = w.threshold if k != 5 else inputs.enclosing_radius(w.dist, n)
+        with R.Rips(w.dist, n, w.dim_max, thr) as g:
+            g.compute()
+            assert 0 < g.device_bytes() <= R.rips_workspace_bytes(n, w.dim_max), (k, n)
