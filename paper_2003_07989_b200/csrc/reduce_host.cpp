@@ -18,13 +18,15 @@ namespace {
 struct Ctx {
     const HostReduceIn& in;
     int M; // vertices of a column simplex
-    explicit Ctx(const HostReduceIn& i) : in(i), M(i.d + 1) {}
-    uint64_t C(int v, int k) const { return in.binom[(size_t)k * in.bstride + v]; }
-    uint32_t key(int a, int b) const
+    std::vector<uint32_t> Kfull; // n x n symmetric copy of the keys (diagonal unused): branch-free, row-contiguous reads
+    explicit Ctx(const HostReduceIn& i) : in(i), M(i.d + 1), Kfull((size_t)i.n * i.n, 0xffffffffu)
     {
-        int hi = a > b ? a : b, lo = a > b ? b : a;
-        return in.K[(size_t)hi * (hi - 1) / 2 + lo];
+        for (int a = 1; a < in.n; ++a)
+            for (int b = 0; b < a; ++b)
+                Kfull[(size_t)a * in.n + b] = Kfull[(size_t)b * in.n + a] = in.K[(size_t)a * (a - 1) / 2 + b];
     }
+    uint64_t C(int v, int k) const { return in.binom[(size_t)k * in.bstride + v]; }
+    uint32_t key(int a, int b) const { return Kfull[(size_t)a * in.n + b]; }
     void decode(uint64_t idx, int m, int* v) const
     { // v[m-1] > ... > v[0]
         int hi = in.n - 1;
@@ -94,15 +96,18 @@ struct Ctx {
         for (int i = 0; i < M; ++i) low[i + 1] = low[i] + C(s[i], i + 1);
         high[M] = 0;
         for (int i = M - 1; i >= 0; --i) high[i] = high[i + 1] + C(s[i], i + 2);
+        const uint32_t* rows[16];
+        for (int j = 0; j < M; ++j) rows[j] = Kfull.data() + (size_t)s[j] * in.n;
         for (int seg = M; seg >= 0; --seg) {
             int hi = (seg == M) ? in.n - 1 : s[seg] - 1;
             int lo = (seg == 0) ? 0 : s[seg - 1] + 1;
+            const uint64_t* Crow = in.binom + (size_t)(seg + 1) * in.bstride;
+            const uint64_t fixed = low[seg] + high[seg];
             for (int v = hi; v >= lo; --v) {
                 uint32_t kt = key_s;
-                for (int j = 0; j < M; ++j) { uint32_t k = key(v, s[j]); if (k < kt) kt = k; }
+                for (int j = 0; j < M; ++j) { uint32_t k = rows[j][v]; if (k < kt) kt = k; }
                 if (kt < in.thr_key) continue;
-                uint64_t t = low[seg] + C(v, seg + 1) + high[seg];
-                h.push(((uint64_t)kt << in.tbits) | t);
+                h.push(((uint64_t)kt << in.tbits) | (fixed + Crow[v]));
             }
         }
         return key_s;
