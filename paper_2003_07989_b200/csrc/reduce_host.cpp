@@ -117,17 +117,19 @@ struct Ctx {
 // Working column of the reduction: a multiset of packed entries (key << tbits | cidx(t)) with "largest
 // first" access.  The pivots of a column come out in (almost always) decreasing order -- whatever an
 // addition brings in lies later in the filtration than the pivot it cancels, except for the unreduced
-// column of an earlier non-apparent owner -- so instead of one big heap the entries are kept in one
-// bucket per key: only the bucket of the current key is a heap (small, cache-resident), the others are
-// plain vectors that are heapified when the sweep reaches them.
+// column of an earlier non-apparent owner -- so instead of one big heap the entries are kept in buckets
+// of neighbouring keys: only the bucket at the sweep position is a heap (small, cache-resident), the
+// others are plain vectors that are heapified when the sweep reaches them.
 class KeyedColumn {
 public:
-    KeyedColumn(uint32_t n_keys, int tbits) : tbits_(tbits), buckets_(n_keys + 1) {}
+    // one bucket per 64 consecutive keys: few enough vectors to stay in cache while a coboundary is pushed
+    KeyedColumn(uint32_t n_keys, int tbits) : tbits_(tbits + 6), buckets_((n_keys >> 6) + 2) {}
     void clear()
     {
         for (uint32_t k : touched_) buckets_[k].clear();
         touched_.clear();
         cur_ = -1;
+        max_key_ = 0;
         size_ = 0;
     }
     void push(uint64_t e)
