@@ -54,8 +54,8 @@ enum {
     RIPS_OK = 0,
     RIPS_EINVAL = -1,    /* bad argument: n < 1, dim_max out of [0,4], NaN/negative/non-finite distance,
                             NaN threshold, d out of range, stage called before its inputs exist */
-    RIPS_EOVERFLOW = -2, /* C(n, dim_max+3) >= 2^63, n >= 65536, or (rank bits + index bits) > 64 so a
-                            column does not fit the packed 64-bit record */
+    RIPS_EOVERFLOW = -2, /* n > 46340 (the n x n key matrix is indexed with 32-bit integers), C(n, dim_max+2) >= 2^62,
+                            or a packed 64-bit record cannot hold (key bits + vertex bits) / (vertex + row bits) */
     RIPS_ENOMEM = -3,    /* device or host allocation failed */
     RIPS_ECUDA = -4      /* CUDA runtime error; text via rips_last_error */
 };

@@ -797,7 +797,8 @@ const char* rips_last_error(void) { return g_last_error.c_str(); }
 
 int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes)
 {
-    if (!bytes || n < 1 || dim_max < 0 || dim_max > 4 || n >= 65536) return RIPS_EINVAL;
+    if (!bytes || n < 1 || dim_max < 0 || dim_max > 4) return RIPS_EINVAL;
+    if (n > 46340) return RIPS_EOVERFLOW;
     std::vector<u64> b;
     build_binom(n, dim_max + 3, b);
     auto C = [&](int k) { return b[(size_t)k * (n + 1) + n]; };
@@ -824,7 +825,7 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     if (!out) return RIPS_EINVAL;
     *out = nullptr;
     if (n < 1 || dim_max < 0 || dim_max > 4 || std::isnan(threshold)) return RIPS_EINVAL;
-    if (n >= 65536) return RIPS_EOVERFLOW;
+    if (n > 46340) return RIPS_EOVERFLOW; // the kernels index the n x n key matrix with 32-bit integers
     if (n > 1 && !dist_lower) return RIPS_EINVAL;
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
