@@ -194,3 +194,44 @@ def test_workspace_estimate_bounds_what_is_held(R):
         with R.Rips(w.dist, n, w.dim_max, thr) as g:
             g.compute()
             assert 0 < g.device_bytes() <= R.rips_workspace_bytes(n, w.dim_max), (k, n)
+
+
+def test_two_contexts_interleaved_and_repeated_stages(R):
+    """Contexts are independent (own streams, own buffers); stages may be repeated in any valid order."""
+    wa, wb = inputs.config(1, 30), inputs.config(3, 28)
+    oa = oracle.barcodes(wa.dist, wa.n, 2, wa.threshold)
+    ob = oracle.barcodes(wb.dist, wb.n, 2, wb.threshold)
+    a = R.Rips(wa.dist, wa.n, 2, wa.threshold)
+    b = R.Rips(wb.dist, wb.n, 2, wb.threshold)
+    a.dim0(); b.dim0()
+    for d in (1, 2):
+        a.stage1(d); b.stage1(d); b.stage2(d); a.stage2(d)
+        a.stage2(d)                       # nothing new to partition: a no-op
+        b.stage1(d); b.stage2(d)          # recomputed from scratch
+        a.reduce(d); b.reduce(d)
+    for g, o in ((a, oa), (b, ob)):
+        for d in (1, 2):
+            pt, ps = g.pivots(d)
+            assert np.array_equal(_np(pt).astype(np.uint64), o[d]["pivot_t"])
+            assert np.array_equal(_np(ps).astype(np.uint64), o[d]["pivot_s"])
+            assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32))
+    a.free(); b.free()
+
+
+def test_import_pivots(R):
+    """rips_import_pivots installs a reduction done elsewhere (here: the oracle's) and rejects unsorted rows."""
+    w = inputs.config(2, 20)
+    o = oracle.barcodes(w.dist, w.n, 2, w.threshold)
+    with R.Rips(w.dist, w.n, 2, w.threshold) as g:
+        g.dim0(); g.stage1(1); g.stage2(1)
+        order = np.argsort(o[1]["red_t"])
+        with pytest.raises(R.RipsError) as e:
+            g.import_pivots(1, o[1]["red_t"][order][::-1], o[1]["red_s"][order][::-1])
+        if o[1]["red_t"].size > 1:
+            assert e.value.code == R.RIPS_EINVAL
+        g.import_pivots(1, o[1]["red_t"][order], o[1]["red_s"][order])
+        pt, ps = g.pivots(1)
+        assert np.array_equal(_np(pt).astype(np.uint64), o[1]["pivot_t"])
+        g.stage1(2); g.stage2(2)
+        fd, fc = g.filtration(2)
+        assert np.array_equal(_np(fc).astype(np.uint64), o[2]["filt_cidx"])
