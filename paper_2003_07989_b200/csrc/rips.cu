@@ -367,7 +367,7 @@ int run_stage1(rips_ctx* c, int d)
     p.clear = cs;
     p.compact = s.compact;
     p.count_only = 0;
-    p.fast_visits = c->fast_visits > 0 ? c->fast_visits : (s.M >= 4 ? 8 : s.M == 3 ? 12 : 16);
+    p.fast_visits = c->fast_visits > 0 ? c->fast_visits : 16; // swept at cfg 2 (4..32): flat above 12
     p.cols_out = p.pairs_out = p.irr_out = p.non_out = nullptr;
     p.irr_cap = p.non_cap = 0;
     p.status = nullptr;
