@@ -235,3 +235,26 @@ def test_import_pivots(R):
         g.stage1(2); g.stage2(2)
         fd, fc = g.filtration(2)
         assert np.array_equal(_np(fc).astype(np.uint64), o[2]["filt_cidx"])
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_randomized_shapes(R, seed):
+    """Seeded random shapes: n, dimension, value regime (distinct reals, heavy ties, clustered points) and
+    threshold all vary; every array against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.integers(5, 70))
+    dim_max = int(rng.integers(1, 4)) if n <= 40 else int(rng.integers(1, 3))
+    regime = seed % 4
+    if regime == 0:
+        low = inputs.random_matrix_lower(n, 50 + seed)
+    elif regime == 1:
+        low = inputs.small_integer_lower(n, 60 + seed, hi=int(rng.integers(2, 9)))
+    elif regime == 2:
+        pts = rng.random((n, 3), dtype=np.float32) * 0.1
+        pts[rng.random(n) < 0.5] += 5.0
+        low = inputs.euclidean_lower(pts)
+    else:
+        low = inputs.euclidean_lower(inputs.cube_points(n, int(rng.integers(1, 5)), 70 + seed))
+    q = float(rng.choice([1.0, 1.0, 0.9, 0.5, 0.2, 0.05]))
+    thr = inf if q == 1.0 else float(np.float32(np.quantile(low, q)))
+    check_against_oracle(R, low, n, dim_max, thr, f"seed {seed}: n={n} dim_max={dim_max} regime={regime} q={q}")
