@@ -30,7 +30,7 @@ namespace {
 
 constexpr int S1_THREADS = 1024;
 constexpr int S1_WARPS = S1_THREADS / 32;
-constexpr int S1_CHUNK = 512;          // most candidates per warp chunk (unit of work and of the look-back chain)
+constexpr int S1_CHUNK = 1024;         // most candidates per warp chunk (unit of work and of the look-back chain)
 constexpr int S1_MAX_FUSED = 3;        // digits of the filtration sort histogrammed on the way out
 constexpr int S1_MAX_FUSED_P = 2;      // digits of the pair partition
 constexpr size_t S1_KF_SMEM_LIMIT = 100 * 1024;  // two blocks per SM
