@@ -1,16 +1,17 @@
 // reduce_host.cpp -- see reduce_host.h.  Implicit cohomology reduction over Z/2 (PAPER.md:127,
-// :168-170, :210) of the columns stage 2 left, with the two-layer pair store of PAPER.md:555-561:
-// pivots found here go to a hash map, apparent pairs are looked up by binary search in the sorted
-// array.  Column entries are packed (key << tbits) | cidx(t); the pivot of a column is the cofacet
-// that comes first in the filtration order (smallest diameter = LARGEST key, then largest cidx,
-// PAPER.md:77-79), i.e. simply the largest packed entry.
+// :168-170, :210) of the non-apparent columns the device could not finish on its own (reduce.cu): those
+// whose pivot, after reduction against the apparent columns, another non-apparent column owns.  Pair
+// store as in PAPER.md:555-561: pivots found here go to a hash map; whether a row belongs to an apparent
+// pair is evaluated from Definition 5 (apparent_lookup) instead of searching the device arrays.  Column
+// entries are packed (key << tbits) | cidx(t); the pivot of a column is the cofacet that comes first in
+// the filtration order (smallest diameter = LARGEST key, then largest cidx), i.e. simply
+// the largest packed entry.
 #include "reduce_host.h"
 
-#include <functional>
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
-
-#include <algorithm>
+#include <functional>
 #include <unordered_map>
 
 namespace {

@@ -1,6 +1,7 @@
-// reduce_host.h -- the serial remainder: reduction of the non-apparent columns (Algorithm 2,
-// PAPER.md:182-200; "submatrix reduction").  NOT the hot path: it runs on the
-// host, as in the paper, and is timed and reported separately (rips_timings).
+// reduce_host.h -- the serial remainder of the reduction of the non-apparent columns (Algorithm 2,
+// PAPER.md:182-200; "submatrix reduction") after the device has reduced every
+// column against the apparent ones (reduce.cu).  NOT the hot path: it runs on the host, as the whole
+// submatrix reduction does in the paper, and is timed and reported separately.
 #pragma once
 #include <stdint.h>
 #include <vector>

@@ -1,7 +1,8 @@
 // rips.cu -- context, per-dimension driver and the C ABI of include/rips.h.
-// Control flow (Fig. 3(b)): dim 0, then per d: stage 1 (clear bitmap ->
-// enumerate/filter/compact -> onesweep sort), stage 2 (apparent kernel with partition -> pair sort),
-// reduction of the few non-apparent columns (host, not hot path), next d.
+// Control flow (Fig. 3(b)): dim 0, then per d: stage 1 (clearing bitmap -> fused
+// enumerate / filter / apparent-test kernel -> onesweep sort of the columns), stage 2 (sorts of the two
+// small lists, stable partition of the pair slots: on side streams, beside stage 1's sort), reduction
+// of the few non-apparent columns (device pre-reduction, serial remainder on the host; not hot path).
 #include "../../include/rips.h"
 
 #include <algorithm>
