@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <functional>
+#include <memory>
 #include <unordered_map>
 
 namespace {
@@ -264,6 +265,56 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
         for (auto& kv : par) if (kv.second) v.push_back(kv.first);
         return vstore[cidx_s] = std::move(v);
     };
+    // Stored reduced columns (the standard form, Algorithm 1; Lemma 3) for
+    // inputs on which restarts keep coming -- flag complexes of random graphs, many equal diameters: the
+    // reduced columns fill in, and both the oblivious form and the V technique re-derive them through
+    // coboundaries again and again.  Once `stored_after` columns have been restarted, every further column
+    // that needs reducing keeps its reduced column R_j (packed entries, first = pivot) and a pivot whose
+    // owner has a stored column costs one pass over that column.  R of an owner finalised before the
+    // switch (or at once, from the device pre-reduction) is computed when first asked for, by reducing it
+    // again against the store -- a pivot of a later column cannot come up, as above.
+    const int64_t stored_after = 16;
+    const int stored_max_depth = 512; // nesting of on-demand recomputations; deeper owners are added as D_i (Algorithm 2)
+    std::unordered_map<uint64_t, std::vector<uint64_t>> rstore; // cidx(s) -> R_s
+    std::vector<std::unique_ptr<Heap>> heaps;                   // one working column per nesting level
+    int64_t n_stored = 0;
+    std::function<uint64_t(uint64_t, int)> reduce_r = [&](uint64_t cidx_s, int depth) -> uint64_t {
+        if ((size_t)depth >= heaps.size()) heaps.emplace_back(new Heap(in.n_keys, in.tbits));
+        Heap& w = *heaps[(size_t)depth];
+        w.clear();
+        cx.push_coboundary(w, cidx_s);
+        for (;;) {
+            uint64_t piv;
+            if (!pop_pivot(w, &piv)) return ~0ull; // a zero column is never an owner: nothing to keep
+            const uint64_t t = piv & tmask;
+            auto it = owner.find(t);
+            if (it == owner.end() || it->second != cidx_s) {
+                if (it != owner.end()) {
+                    const uint64_t own = it->second;
+                    auto rs = rstore.find(own);
+                    if (rs == rstore.end() && depth < stored_max_depth) {
+                        reduce_r(own, depth + 1);
+                        rs = rstore.find(own);
+                    }
+                    w.push(piv); // the added column holds t as well: the two cancel
+                    if (rs != rstore.end()) for (uint64_t e : rs->second) w.push(e);
+                    else cx.push_coboundary(w, own);
+                    ++out.additions;
+                    continue;
+                }
+                uint64_t s2 = 0;
+                if (cx.apparent_lookup(t, &s2)) { w.push(piv); cx.push_coboundary(w, s2); ++out.additions; continue; }
+            }
+            // a new pivot, or the one this column is already known to own: keep the reduced column
+            std::vector<uint64_t> r;
+            r.push_back(piv);
+            uint64_t e;
+            while (pop_pivot(w, &e)) r.push_back(e);
+            rstore[cidx_s] = std::move(r);
+            ++n_stored;
+            return piv;
+        }
+    };
     const int64_t oblivious_budget = 256; // additions before a column is restarted with the V technique
     int64_t n_fast = 0, n_slow = 0, n_def = 0, n_own_adds = 0;
     Heap h(in.n_keys, in.tbits);
@@ -283,6 +334,16 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
             if (owner.find(piv & tmask) == owner.end()) { finalize(j, piv, cidx_s, key_s); ++n_fast; continue; }
         }
         ++n_slow;
+        if (n_vmode >= stored_after) {
+            const uint64_t pv = reduce_r(cidx_s, 0);
+            if (pv == ~0ull) {
+                out.ess_s.push_back(cidx_s);
+                out.ess_key.push_back(key_s);
+                out.ess_col.push_back(j);
+            } else
+                finalize(j, pv, cidx_s, key_s);
+            continue;
+        }
         const int64_t adds0 = out.additions;
         h.clear();
         cx.push_coboundary(h, cidx_s);
@@ -322,6 +383,6 @@ void host_reduce_columns(const HostReduceIn& in, HostReduceOut& out)
         }
     }
     if (getenv("RIPS_DEBUG"))
-        fprintf(stderr, "host_reduce d=%d: cols %lld final at once %lld reduced here %lld (not pre-reduced %lld), additions of reduced columns %lld, restarted with V %lld\n", in.d,
-                (long long)in.ncols, (long long)n_fast, (long long)n_slow, (long long)n_def, (long long)n_own_adds, (long long)n_vmode);
+        fprintf(stderr, "host_reduce d=%d: cols %lld final at once %lld reduced here %lld (not pre-reduced %lld), additions of reduced columns %lld, restarted with V %lld, reduced columns stored %lld\n", in.d,
+                (long long)in.ncols, (long long)n_fast, (long long)n_slow, (long long)n_def, (long long)n_own_adds, (long long)n_vmode, (long long)n_stored);
 }
