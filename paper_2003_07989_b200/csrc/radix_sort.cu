@@ -9,11 +9,20 @@
 
 namespace {
 
-constexpr int SORT_THREADS = 384;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
-constexpr int SORT_IPT = 12;
-constexpr int SORT_MIN_BLOCKS = 3;
-constexpr int SORT_LB_BATCH = 8;     // predecessor tiles read per look-back step
-constexpr int SORT_RANK_BATCH = 3;   // records ranked per pipelined batch (divides SORT_IPT)
+#ifndef RIPS_SORT_THREADS
+#define RIPS_SORT_THREADS 256
+#define RIPS_SORT_IPT 20
+#define RIPS_SORT_MIN_BLOCKS 3
+#define RIPS_SORT_RANK_BATCH 2
+#endif
+constexpr int SORT_THREADS = RIPS_SORT_THREADS;   // >= RIPS_SORT_MAX_BINS: one thread per bin for the scans and the look-back
+constexpr int SORT_IPT = RIPS_SORT_IPT;
+constexpr int SORT_MIN_BLOCKS = RIPS_SORT_MIN_BLOCKS;
+#ifndef RIPS_SORT_LB_BATCH
+#define RIPS_SORT_LB_BATCH 8
+#endif
+constexpr int SORT_LB_BATCH = RIPS_SORT_LB_BATCH;     // predecessor tiles read per look-back step
+constexpr int SORT_RANK_BATCH = RIPS_SORT_RANK_BATCH;   // records ranked per pipelined batch (divides SORT_IPT)
 constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 
@@ -92,7 +101,7 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 // look-back at once, scan over the bins; (4) records placed in tile-sorted order in shared memory;
 // (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
-template <bool MATCH>
+template <bool MATCH, bool EARLY>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
                      const u64* __restrict__ global_base, u64* status, u32* ticket)
@@ -104,6 +113,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     u64* goff = stage + SORT_TILE;                                        // [MAX_BINS]
     u32* whist = reinterpret_cast<u32*>(goff + RIPS_SORT_MAX_BINS);       // [SORT_WARPS][MAX_BINS]
     u32* bin_start = whist + SORT_WARPS * RIPS_SORT_MAX_BINS;             // [MAX_BINS]
+    u32* thist = bin_start + RIPS_SORT_MAX_BINS;                          // [MAX_BINS] (EARLY only)
     __shared__ u32 s_tile;
     __shared__ u32 s_wsum[8];
 
@@ -112,6 +122,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     u32* wh = whist + warp * RIPS_SORT_MAX_BINS;
 #pragma unroll
     for (int i = lane; i < RIPS_SORT_MAX_BINS; i += 32) wh[i] = 0;
+    if (EARLY && tid < RIPS_SORT_MAX_BINS) thist[tid] = 0;
     __syncthreads();
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
@@ -128,6 +139,27 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
         for (int i = 0; i < SORT_IPT; ++i) {
             i64 idx = wbase + i * 32;
             key[i] = idx < n ? __ldcs(in + idx) : ~0ull; // padding: last bin, last inside the tile, never written
+        }
+    }
+
+    // ---- (1b) EARLY: the tile's digit counts by plain shared atomics, published for the look-back
+    // before the ranking, so that the tiles behind this one never wait for its ranking (the ranking
+    // is the longest phase of a tile; the look-back below then finds every predecessor published).
+    if (EARLY) {
+#pragma unroll
+        for (int i = 0; i < SORT_IPT; ++i) {
+            const u32 d = (u32)(key[i] >> shift) & mask;
+            const u32 d0 = __shfl_sync(RIPS_FULL_MASK, d, 0);
+            if (__all_sync(RIPS_FULL_MASK, d == d0)) { // skewed digits: one add per warp instead of 32 serialised ones
+                if (lane == 0) atomicAdd(&thist[d0], 32u);
+            } else {
+                atomicAdd(&thist[d], 1u);
+            }
+        }
+        __syncthreads();
+        if (tid < nbins) {
+            const u32 c = thist[tid] - ((tid == nbins - 1) ? (u32)(SORT_TILE - count) : 0u);
+            st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)c);
         }
     }
 
@@ -189,7 +221,8 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
                 run += c;
             }
             my_count = (tid == nbins - 1) ? run - (u32)n_pad : run;
-            st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
+            if (!EARLY)
+                st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
         }
         // block scan of `run` over the first MAX_BINS threads (8 warps)
         u32 incl = run;
@@ -274,7 +307,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
 size_t pass_smem_bytes(int)
 {
     const size_t nb = RIPS_SORT_MAX_BINS;
-    return (size_t)SORT_TILE * 8 + nb * 8 + (size_t)SORT_WARPS * nb * 4 + nb * 4;
+    return (size_t)SORT_TILE * 8 + nb * 8 + (size_t)SORT_WARPS * nb * 4 + nb * 4 + nb * 4;
 }
 
 struct ScratchLayout {
@@ -336,18 +369,20 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     }
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)pass_smem_bytes(8));
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(onesweep_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)pass_smem_bytes(8));
-        if (e != cudaSuccess) return e;
+        cudaError_t e = cudaSuccess;
+        const void* fns[4] = {(const void*)onesweep_pass_kernel<true, false>, (const void*)onesweep_pass_kernel<false, false>,
+                              (const void*)onesweep_pass_kernel<true, true>, (const void*)onesweep_pass_kernel<false, true>};
+        for (int f = 0; f < 4; ++f) {
+            e = cudaFuncSetAttribute(fns[f], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
+            if (e != cudaSuccess) return e;
+        }
         e = cudaFuncSetAttribute(sort_histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 4);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     static const int force_rank = getenv("RIPS_SORT_RANK") ? atoi(getenv("RIPS_SORT_RANK")) : 1; // tuning: 0 ballots, 1 match
+    static const int early = getenv("RIPS_SORT_EARLY") ? atoi(getenv("RIPS_SORT_EARLY")) : 0; // tuning: 0 publish after the ranking
     if (force_rank >= 0) skewed_digits = force_rank != 0;
     ScratchLayout L = scratch_layout(n, plan);
     unsigned char* sc = (unsigned char*)scratch;
@@ -380,12 +415,12 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         size_t status_bytes = (size_t)tiles * ((size_t)1 << plan.bits[p]) * 8;
         e = cudaMemsetAsync(status, 0, status_bytes, stream);
         if (e != cudaSuccess) return e;
-        if (skewed_digits)
-            onesweep_pass_kernel<true><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-                src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p);
-        else
-            onesweep_pass_kernel<false><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-                src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p);
+#define RIPS_SORT_LAUNCH(M, E)                                                                                      \
+    onesweep_pass_kernel<M, E><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(          \
+        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p)
+        if (skewed_digits) { if (early) RIPS_SORT_LAUNCH(true, true); else RIPS_SORT_LAUNCH(true, false); }
+        else               { if (early) RIPS_SORT_LAUNCH(false, true); else RIPS_SORT_LAUNCH(false, false); }
+#undef RIPS_SORT_LAUNCH
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }
