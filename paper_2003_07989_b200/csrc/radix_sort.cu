@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 template <bool MATCH, bool EARLY>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
-                     const u64* __restrict__ global_base, u64* status, u32* ticket)
+                     const u64* __restrict__ global_base, u64* status, u32* ticket, int pf_dist)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nbins = 1 << bits;
@@ -127,6 +127,18 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
     const int count = (int)min((i64)SORT_TILE, n - base);
+
+    // L2 prefetch of the tile that is pf_dist tickets ahead (one bulk instruction): a CTA has loads in flight only
+    // during its short load phase, so without it DRAM reads come in bursts; with it the later loads hit L2.
+    if (tid == 0 && pf_dist > 0) {
+        const i64 pbase = (tile + pf_dist) * SORT_TILE;
+        if (pbase < n) {
+            const u32 bytes = (u32)(min((i64)SORT_TILE, n - pbase) * 8) & ~15u;
+            const u64* src = in + pbase;
+            if (bytes && ((unsigned long long)src & 15ull) == 0)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+        }
+    }
 
     // ---- (1) load: item i of lane l of warp w is record base + w*32*IPT + i*32 + l
     u64 key[SORT_IPT];
@@ -383,6 +395,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     }
     static const int force_rank = getenv("RIPS_SORT_RANK") ? atoi(getenv("RIPS_SORT_RANK")) : 1; // tuning: 0 ballots, 1 match
     static const int early = getenv("RIPS_SORT_EARLY") ? atoi(getenv("RIPS_SORT_EARLY")) : 0; // tuning: 0 publish after the ranking
+    static const int pf_dist = getenv("RIPS_SORT_PF") ? atoi(getenv("RIPS_SORT_PF")) : 148; // tuning: tiles ahead, 0 = off
     if (force_rank >= 0) skewed_digits = force_rank != 0;
     ScratchLayout L = scratch_layout(n, plan);
     unsigned char* sc = (unsigned char*)scratch;
@@ -417,7 +430,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         if (e != cudaSuccess) return e;
 #define RIPS_SORT_LAUNCH(M, E)                                                                                      \
     onesweep_pass_kernel<M, E><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(          \
-        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p)
+        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist)
         if (skewed_digits) { if (early) RIPS_SORT_LAUNCH(true, true); else RIPS_SORT_LAUNCH(true, false); }
         else               { if (early) RIPS_SORT_LAUNCH(false, true); else RIPS_SORT_LAUNCH(false, false); }
 #undef RIPS_SORT_LAUNCH
