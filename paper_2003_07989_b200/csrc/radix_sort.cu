@@ -267,31 +267,38 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
         u64 excl = 0;
         if (tile > 0) {
             i64 t = tile - 1;
-            bool done = false;
-            while (!done) {
+            const u64* sp = status + t * nbins + tid; // status word of tile t and this bin; one tile back = -nbins words
+            while (true) {
                 // wait (one word, with a back-off) until the nearest tile not yet summed is published; the
                 // tiles before it are older and almost always published already, so they are read as a batch
-                u64 s0 = ld_volatile_u64(status + t * nbins + tid);
+                u64 s0 = ld_volatile_u64(sp);
                 while ((s0 >> 62) == 0) {
                     __nanosleep(40);
-                    s0 = ld_volatile_u64(status + t * nbins + tid);
+                    s0 = ld_volatile_u64(sp);
                 }
                 excl += s0 & LB_VALUE_MASK;
+                sp -= nbins;
                 --t;
                 if ((s0 >> 62) == 2 || t < 0) break;
-                u64 sv[SORT_LB_BATCH];
+                if (t >= SORT_LB_BATCH) { // the whole batch lies at tiles >= 1: no bound checks inside
+                    u64 sv[SORT_LB_BATCH];
+                    const u64* q = sp;
 #pragma unroll
-                for (int b = 0; b < SORT_LB_BATCH; ++b)
-                    sv[b] = (t - b >= 0) ? ld_volatile_u64(status + (t - b) * nbins + tid) : LB_FLAG_INC;
+                    for (int b = 0; b < SORT_LB_BATCH; ++b) {
+                        sv[b] = ld_volatile_u64(q);
+                        q -= nbins;
+                    }
+                    bool fin = false;
 #pragma unroll
-                for (int b = 0; b < SORT_LB_BATCH; ++b) {
-                    if (!done) {
-                        const u64 flag = sv[b] >> 62;
+                    for (int b = 0; b < SORT_LB_BATCH; ++b) {
+                        const u32 flag = (u32)(sv[b] >> 62);
                         if (flag == 0) break; // not published yet: wait for this tile
                         excl += sv[b] & LB_VALUE_MASK;
+                        sp -= nbins;
                         --t;
-                        if (flag == 2 || t < 0) done = true;
+                        if (flag == 2) { fin = true; break; }
                     }
+                    if (fin) break;
                 }
             }
             st_volatile_u64(status + tile * nbins + tid, LB_FLAG_INC | (excl + (u64)my_count));
