@@ -111,7 +111,10 @@ def test_sort_primitive(R):
     import torch
     rng = np.random.default_rng(11)
     for n, lo, hi in [(1, 0, 8), (2, 3, 20), (1000, 0, 64), (8192, 5, 22), (8193, 0, 9), (100003, 13, 30),
-                      (1 << 20, 40, 57), (300007, 0, 1)]:
+                      (1 << 20, 40, 57), (300007, 0, 1),
+                      # around the tile of 256 x 20 records and the look-back batch of 8 tiles
+                      (5119, 0, 8), (5120, 2, 10), (5121, 0, 16), (5120 * 9, 7, 15), (5120 * 10 + 1, 0, 15),
+                      (5120 * 17 - 1, 20, 27), (3000017, 3, 19)]:
         a = rng.integers(0, 1 << 63, n, dtype=np.int64) * 2 + rng.integers(0, 2, n, dtype=np.int64)
         if n == 100003:
             a[:] = a[0]                       # all keys equal: must come back untouched (stability)
