@@ -118,7 +118,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     __shared__ u32 s_wsum[8];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    if (tid == 0) s_tile = ticket ? atomicAdd(ticket, 1u) : blockIdx.x;
     u32* wh = whist + warp * RIPS_SORT_MAX_BINS;
 #pragma unroll
     for (int i = lane; i < RIPS_SORT_MAX_BINS; i += 32) wh[i] = 0;
@@ -402,6 +402,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     }
     static const int force_rank = getenv("RIPS_SORT_RANK") ? atoi(getenv("RIPS_SORT_RANK")) : 1; // tuning: 0 ballots, 1 match
     static const int early = getenv("RIPS_SORT_EARLY") ? atoi(getenv("RIPS_SORT_EARLY")) : 0; // tuning: 0 publish after the ranking
+    static const int use_ticket = getenv("RIPS_SORT_TICKET") ? atoi(getenv("RIPS_SORT_TICKET")) : 1; // measurement only: 0 = tile from blockIdx.x
     static const int pf_dist = getenv("RIPS_SORT_PF") ? atoi(getenv("RIPS_SORT_PF")) : 148; // tuning: tiles ahead, 0 = off
     if (force_rank >= 0) skewed_digits = force_rank != 0;
     ScratchLayout L = scratch_layout(n, plan);
@@ -437,7 +438,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         if (e != cudaSuccess) return e;
 #define RIPS_SORT_LAUNCH(M, E)                                                                                      \
     onesweep_pass_kernel<M, E><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(          \
-        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist)
+        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, use_ticket ? ticket + p : (u32*)nullptr, pf_dist)
         if (skewed_digits) { if (early) RIPS_SORT_LAUNCH(true, true); else RIPS_SORT_LAUNCH(true, false); }
         else               { if (early) RIPS_SORT_LAUNCH(false, true); else RIPS_SORT_LAUNCH(false, false); }
 #undef RIPS_SORT_LAUNCH
