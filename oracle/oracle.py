@@ -58,6 +58,7 @@ def lib():
         _lib.oracle_reduce.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_void_p, C.c_int64,
                                        C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(u64p), C.POINTER(u64p),
                                        i64p, C.POINTER(u64p), i64p, i64p]
+        _lib.oracle_reduce_explicit.argtypes = _lib.oracle_reduce.argtypes
     return _lib
 
 
@@ -157,14 +158,17 @@ def dim0(dist, n, threshold=inf):
             "n_components": ncomp.value}
 
 
-def reduce_columns(dist, n, d, threshold, col_cidx, known_t=(), known_s=()):
-    """Algorithm 2 over the given columns (coboundary order).  Returns dict: t, s (pivots in processing
-    order), essential (cidx of zero columns), additions."""
+def reduce_columns(dist, n, d, threshold, col_cidx, known_t=(), known_s=(), explicit=False):
+    """The reduction over the given columns (coboundary order).  Returns dict: t, s (pivots in processing
+    order), essential (cidx of zero columns), additions.  explicit=False: implicit columns, working column a
+    heap (oracle_reduce); explicit=True: Algorithm 1 on the explicit coboundary matrix, working column a bit
+    array over all rows (oracle_reduce_explicit) -- the same pairs, for inputs whose reduced columns fill in."""
     dist, col_cidx = _f32(dist), _u64(col_cidx)
     known_t, known_s = _u64(known_t), _u64(known_s)
     pt, ps, pe = u64p(), u64p(), u64p()
     npiv, ness, adds = C.c_int64(), C.c_int64(), C.c_int64()
-    lib().oracle_reduce(_ptr(dist), n, d, threshold, _ptr(col_cidx), col_cidx.size, _ptr(known_t),
+    fn = lib().oracle_reduce_explicit if explicit else lib().oracle_reduce
+    fn(_ptr(dist), n, d, threshold, _ptr(col_cidx), col_cidx.size, _ptr(known_t),
                         _ptr(known_s), known_t.size, C.byref(pt), C.byref(ps), C.byref(npiv), C.byref(pe),
                         C.byref(ness), C.byref(adds))
     # the three arrays were allocated with ncols entries each; copy the used prefix
@@ -174,7 +178,7 @@ def reduce_columns(dist, n, d, threshold, col_cidx, known_t=(), known_s=()):
     return {"t": t, "s": s, "essential": e, "additions": adds.value}
 
 
-def barcodes(dist, n, dim_max, threshold=inf, use_apparent=True, upto_stage2_dim=None):
+def barcodes(dist, n, dim_max, threshold=inf, use_apparent=True, explicit=False):
     """The whole pipeline.  Returns dict d -> dict with every exposed array:
 
       d = 0:  pivot_t, pivot_s (ascending t), bars
@@ -197,11 +201,11 @@ def barcodes(dist, n, dim_max, threshold=inf, use_apparent=True, upto_stage2_dim
         fd, fc, counts = stage1(dist, n, d, threshold, cleared)
         s2 = stage2(dist, n, d, fd, fc)
         if use_apparent:
-            red = reduce_columns(dist, n, d, threshold, s2["non_cidx"], s2["app_t"], s2["app_s"])
+            red = reduce_columns(dist, n, d, threshold, s2["non_cidx"], s2["app_t"], s2["app_s"], explicit)
             all_t = np.concatenate([s2["app_t"], red["t"]])
             all_s = np.concatenate([s2["app_s"], red["s"]])
         else:
-            red = reduce_columns(dist, n, d, threshold, fc)
+            red = reduce_columns(dist, n, d, threshold, fc, explicit=explicit)
             all_t, all_s = red["t"], red["s"]
         order = np.argsort(all_t, kind="stable")
         piv_t, piv_s = all_t[order], all_s[order]

@@ -24,6 +24,10 @@
  *                  Algorithm 2; the reduced columns are kept because the oblivious
  *                  form, which re-adds D_i, needs orders of magnitude more additions on "difficult"
  *                  inputs such as config 3's random matrices.
+ *   oracle_reduce_explicit  the same reduction as Algorithm 1 verbatim on the explicit
+ *                  coboundary matrix (rows ranked in reverse filtration order, working column a bit
+ *                  array, R_j <- R_j + R_i an exclusive or): same pairs; used where the heap of
+ *                  oracle_reduce is too slow (config 3, dimension 1).
  *
  * No blocking, fusion or reordering beyond what those passages state.  The only concession to
  * run time is `#pragma omp parallel for` over independent simplices (Corollary 8)
@@ -545,6 +549,122 @@ int oracle_reduce(const float *D, int n, int d, float threshold, const u64 *col_
     for (i64 j = 0; j < ncols; ++j) free(Rcol[j]);
     free(Rcol); free(Rlen);
     free(h.a); free(map.k); free(map.v);
+    binom_free(&b);
+    *piv_t = pt; *piv_s = ps; *n_piv = np; *ess_s = es; *n_ess = ne;
+    if (additions) *additions = adds;
+    return 0;
+}
+
+/* ------------------------------------------------------------------ O3b: Algorithm 1 on explicit columns */
+
+/* A second, plainer reduction for inputs on which the reduced columns fill in ("difficult datasets",
+ * PAPER.md:210; config 3's random matrices): the standard persistence algorithm, Algorithm 1
+ * (PAPER.md:99-121), on the EXPLICIT coboundary matrix.  Rows = the
+ * (d+1)-simplices of diameter <= threshold, indexed like the matrix of PAPER.md:127 in the reverse of the
+ * filtration order (diameter descending, cidx ascending: the comparator of stage 1), so that low(R_j),
+ * the largest row index of a nonzero entry, is the cofacet that comes FIRST in the filtration order.  The
+ * working column R_j is a bit array over the rows, R_j <- R_j + R_i is an exclusive or; the reduced
+ * columns are kept as lists of row indices.  Same interface and same (unique) pairs as oracle_reduce;
+ * memory = one word per possible row (the index of cidx -> row) + the stored columns. */
+int oracle_reduce_explicit(const float *D, int n, int d, float threshold, const u64 *col_cidx, i64 ncols,
+                           const u64 *known_t, const u64 *known_s, i64 n_known,
+                           u64 **piv_t, u64 **piv_s, i64 *n_piv, u64 **ess_s, i64 *n_ess, i64 *additions)
+{
+    int m = d + 1;
+    binom_t b;
+    binom_init(&b, n, d + 2);
+    /* rows: every (d+1)-simplex within the threshold, in coboundary order */
+    u64 total_rows = C(&b, n, d + 2);
+    col_t *rows = (col_t *)malloc(sizeof(col_t) * (total_rows ? total_rows : 1));
+    i64 nrows = 0;
+    for (u64 idx = 0; idx < total_rows; ++idx) {
+        int verts[MAXV + 1];
+        decode(&b, idx, m + 1, n, verts);
+        float x = diameter(D, verts, m + 1);
+        if (x <= threshold) { rows[nrows].diam = x; rows[nrows].cidx = idx; ++nrows; }
+    }
+    qsort(rows, (size_t)nrows, sizeof(col_t), cmp_coboundary_order);
+    i64 *row_of = (i64 *)malloc(sizeof(i64) * (total_rows ? total_rows : 1)); /* cidx(t) -> row index, -1 = above the threshold */
+    for (u64 i = 0; i < total_rows; ++i) row_of[i] = -1;
+    for (i64 r = 0; r < nrows; ++r) row_of[rows[r].cidx] = r;
+    i64 nwords = (nrows + 63) / 64 + 1;
+    u64 *w = (u64 *)calloc((size_t)nwords, sizeof(u64));           /* the working column R_j */
+    i64 *owner = (i64 *)malloc(sizeof(i64) * (nrows ? nrows : 1)); /* lookup[row] = j, -1 = none (Alg. 1 line 1) */
+    for (i64 r = 0; r < nrows; ++r) owner[r] = -1;
+    i64 **Rcol = (i64 **)calloc((size_t)(ncols ? ncols : 1), sizeof(i64 *));
+    i64 *Rlen = (i64 *)calloc((size_t)(ncols ? ncols : 1), sizeof(i64));
+    u64 *pt = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
+    u64 *ps = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
+    u64 *es = (u64 *)malloc(sizeof(u64) * (ncols ? ncols : 1));
+    i64 np = 0, ne = 0, adds = 0;
+    int V[MAXV], T[MAXV + 1];
+    for (i64 j = 0; j < ncols; ++j) {
+        /* R_j <- D_j: the coboundary of the column's simplex */
+        i64 top = -1; /* no bit is set above row `top` */
+#define XOR_COBOUNDARY(CIDX)                                                                     \
+        do {                                                                                     \
+            decode(&b, (CIDX), m, n, V);                                                         \
+            for (int v = 0; v < n; ++v) {                                                        \
+                int in_s = 0;                                                                    \
+                for (int p = 0; p < m; ++p) in_s |= (V[p] == v);                                 \
+                if (in_s) continue;                                                              \
+                int q = 0, placed = 0;                                                           \
+                for (int p = 0; p < m; ++p) {                                                    \
+                    if (!placed && v > V[p]) { T[q++] = v; placed = 1; }                         \
+                    T[q++] = V[p];                                                               \
+                }                                                                                \
+                if (!placed) T[q++] = v;                                                         \
+                i64 r = row_of[encode(&b, T, m + 1)];                                            \
+                if (r < 0) continue; /* cofacet above the threshold (reading R15) */             \
+                w[r >> 6] ^= 1ull << (r & 63);                                                   \
+                if (r > top) top = r;                                                            \
+            }                                                                                    \
+        } while (0)
+        XOR_COBOUNDARY(col_cidx[j]);
+        for (;;) {
+            /* low(R_j): the largest row index with a nonzero entry */
+            i64 low = -1;
+            for (i64 wd = top >> 6; top >= 0 && wd >= 0; --wd)
+                if (w[wd]) {
+                    int bit = 63;
+                    while (!((w[wd] >> bit) & 1)) --bit;
+                    low = wd * 64 + bit;
+                    break;
+                }
+            top = low;
+            if (low < 0) { es[ne++] = col_cidx[j]; break; }                       /* zero column */
+            if (owner[low] >= 0) {                                                /* R_j <- R_j + R_i, i = lookup[low] */
+                i64 i = owner[low];
+                for (i64 e = 0; e < Rlen[i]; ++e) w[Rcol[i][e] >> 6] ^= 1ull << (Rcol[i][e] & 63);
+                ++adds;
+                continue;
+            }
+            int found = 0;
+            u64 s2 = 0;
+            if (n_known) {                                                        /* an apparent column: R_i = D_i */
+                u64 ct = rows[low].cidx;
+                i64 lo = 0, hi = n_known;
+                while (lo < hi) { i64 mid = lo + (hi - lo) / 2; if (known_t[mid] < ct) lo = mid + 1; else hi = mid; }
+                if (lo < n_known && known_t[lo] == ct) { found = 1; s2 = known_s[lo]; }
+            }
+            if (found) { XOR_COBOUNDARY(s2); top = low; ++adds; continue; }
+            owner[low] = j;                                                       /* lookup[low(R_j)] <- j */
+            pt[np] = rows[low].cidx; ps[np] = col_cidx[j]; ++np;
+            i64 cnt = 0;
+            for (i64 wd = 0; wd <= (low >> 6); ++wd) cnt += __builtin_popcountll(w[wd]);
+            Rcol[j] = (i64 *)malloc(sizeof(i64) * (size_t)cnt);
+            for (i64 wd = low >> 6; wd >= 0; --wd)                                /* keep R_j, clear the working column */
+                while (w[wd]) {
+                    int bit = 63 - __builtin_clzll(w[wd]);
+                    Rcol[j][Rlen[j]++] = wd * 64 + bit;
+                    w[wd] &= ~(1ull << bit);
+                }
+            break;
+        }
+#undef XOR_COBOUNDARY
+    }
+    for (i64 j = 0; j < ncols; ++j) free(Rcol[j]);
+    free(Rcol); free(Rlen); free(owner); free(w); free(row_of); free(rows);
     binom_free(&b);
     *piv_t = pt; *piv_s = ps; *n_piv = np; *ess_s = es; *n_ess = ne;
     if (additions) *additions = adds;

@@ -172,6 +172,93 @@ def test_P13_c_oracle_equals_brute_force(n, dim_max):
                         assert o_app[d]["essential"].size == 0
 
 
+@pytest.mark.parametrize("n,dim_max", [(3, 2), (6, 3), (8, 2), (9, 1)])
+def test_P13_explicit_reduction_equals_brute_force(n, dim_max):
+    """oracle_reduce_explicit (Algorithm 1 on the explicit coboundary matrix) against the
+    brute-force boundary-matrix reduction, with and without the apparent pairs as known pivots."""
+    for seed in range(3):
+        for name, low in _regimes(n, seed):
+            for thr in (inf, float(np.float32(np.quantile(low, 0.6)))):
+                b = brute.persistence(low, n, dim_max, thr)
+                for use_apparent in (True, False):
+                    o = oracle.barcodes(low, n, dim_max, thr, use_apparent=use_apparent, explicit=True)
+                    for d in range(1, dim_max + 1):
+                        got = sorted(zip((int(x) for x in o[d]["pivot_s"]), (int(x) for x in o[d]["pivot_t"])))
+                        assert got == b[d]["pairs"], (name, thr, d, use_apparent)
+                        assert bars_sorted(o[d]["bars"]) == b[d]["bars"], (name, thr, d, use_apparent)
+                        assert sorted(int(x) for x in o[d]["essential"]) == b[d]["essential"]
+
+
+@pytest.mark.parametrize("k,n", [(1, 26), (2, 22), (3, 30), (4, 40), (5, 28)])
+def test_explicit_and_heap_reductions_agree(k, n):
+    """The two reductions of the oracle (implicit columns + heap; explicit matrix + bit array) on the shadow
+    configs: same pivots in the same processing order, same essential columns."""
+    w = inputs.config(k, n)
+    thr = w.threshold if k not in (4, 5) else (inputs.enclosing_radius(w.dist, n) if k == 5 else float(np.float32(np.quantile(w.dist, 0.3))))
+    a = oracle.barcodes(w.dist, n, w.dim_max, thr)
+    e = oracle.barcodes(w.dist, n, w.dim_max, thr, explicit=True)
+    for d in range(1, w.dim_max + 1):
+        for key in ("red_t", "red_s", "essential", "pivot_t", "pivot_s"):
+            assert np.array_equal(a[d][key], e[d][key]), (d, key)
+        assert np.array_equal(a[d]["bars"].view(np.uint32), e[d]["bars"].view(np.uint32))
+
+
+# ---------------------------------------------------------------- the slice mode of stage 1, the visit counts of stage 2
+
+@pytest.mark.parametrize("k,n,d", [(1, 20, 2), (2, 16, 3), (3, 24, 1), (4, 30, 2), (5, 18, 2)])
+def test_stage1_slices_concatenate_to_the_whole(k, n, d):
+    """oracle_stage1 with idx_lo/idx_hi and do_sort = 0 (what the full-size GPU tests and bench.py call): the
+    survivors of consecutive slices, concatenated, are the survivors of the whole index range in increasing
+    cidx, and re-sorted they are the filtration array; against the definition (brute.coboundary_columns)."""
+    w = inputs.config(k, n)
+    thr = inf if k not in (4, 5) else float(np.float32(np.quantile(w.dist, 0.5)))
+    prev = oracle.barcodes(w.dist, n, d - 1, thr) if d > 1 else {0: oracle.barcodes(w.dist, n, 0, thr)[0]}
+    cleared = prev[d - 1]["pivot_t"]
+    total = comb(n, d + 1)
+    fd, fc, counts = oracle.stage1(w.dist, n, d, thr, cleared)                    # whole range, sorted
+    ud, uc, ucounts = oracle.stage1(w.dist, n, d, thr, cleared, sort=False)        # whole range, cidx order
+    assert ucounts == counts and list(uc) == sorted(int(c) for c in fc)
+    cuts = [0, 1, total // 7, total // 7 + 1, total // 2, total - 3, total]
+    cd, cc, tot = [], [], {"kept": 0, "removed_by_diameter": 0, "cleared": 0}
+    for lo, hi in zip(cuts[:-1], cuts[1:]):
+        sd, sc, c = oracle.stage1(w.dist, n, d, thr, cleared, lo, hi, sort=False)
+        assert all(lo <= int(x) < hi for x in sc)
+        assert c["kept"] + c["removed_by_diameter"] + c["cleared"] == hi - lo
+        cd.append(sd); cc.append(sc)
+        for key in tot:
+            tot[key] += c[key]
+    cd, cc = np.concatenate(cd), np.concatenate(cc)
+    assert tot == counts
+    assert np.array_equal(cc, uc) and np.array_equal(cd.view(np.uint32), ud.view(np.uint32))
+    # against the definition: brute force columns (coboundary order), re-sorted by cidx
+    if n <= 20:
+        b = brute.persistence(w.dist, n, d - 1, thr) if d > 1 else brute.persistence(w.dist, n, 0, thr)
+        want = brute.coboundary_columns(w.dist, n, d, thr, [t for (_, t) in b[d - 1]["pairs"]])
+        assert sorted((c, dm) for dm, c in want) == list(zip((int(x) for x in cc), (float(x) for x in cd)))
+    # an empty slice and a slice of one
+    sd, sc, c = oracle.stage1(w.dist, n, d, thr, cleared, 5, 5, sort=False)
+    assert sc.size == 0 and c == {"kept": 0, "removed_by_diameter": 0, "cleared": 0}
+
+
+@pytest.mark.parametrize("k,n,d", [(1, 18, 1), (2, 14, 2), (3, 20, 1), (3, 12, 3)])
+def test_stage2_visit_counts(k, n, d):
+    """oracle_stage2's `visits` output: the number of cofacets evaluated per column = position (counted over
+    the vertices not in s, from n-1 down) of the first cofacet of equal diameter, or n-d-1 if there is none;
+    re-derived with numpy from the square matrix."""
+    w = inputs.config(k, n)
+    sq = inputs.square_from_lower(w.dist, n)
+    fd, fc, _ = oracle.stage1(w.dist, n, d)
+    s2 = oracle.stage2(w.dist, n, d, fd, fc, want_visits=True)
+    for i in range(fc.size):
+        verts = oracle.decode(int(fc[i]), d + 1, n)
+        others = [v for v in range(n - 1, -1, -1) if v not in verts]
+        dt = np.maximum(fd[i], sq[np.ix_(others, verts)].max(axis=1))
+        hit = np.nonzero(dt == fd[i])[0]
+        assert s2["visits"][i] == (hit[0] + 1 if hit.size else n - d - 1)
+        if not hit.size:
+            assert s2["flag"][i] == 0
+
+
 @pytest.mark.parametrize("n,d", [(6, 1), (7, 2), (8, 1), (8, 3)])
 def test_P7_apparent_set_unchanged_by_clearing(n, d):
     """Proposition 10: Alg. 3 over ALL d-simplices finds the same pairs as over the cleared columns."""
