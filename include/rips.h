@@ -56,7 +56,7 @@ enum {
                             NaN threshold, d out of range, stage called before its inputs exist */
     RIPS_EOVERFLOW = -2, /* n > 46340 (the n x n key matrix is indexed with 32-bit integers), C(n, dim_max+2) >= 2^62,
                             or a packed 64-bit record cannot hold (key bits + vertex bits) / (vertex + row bits) */
-    RIPS_ENOMEM = -3,    /* device or host allocation failed */
+    RIPS_ENOMEM = -3,    /* the workspace is too small (rips_last_required_bytes), or an allocation failed */
     RIPS_ECUDA = -4      /* CUDA runtime error; text via rips_last_error */
 };
 
@@ -77,6 +77,10 @@ typedef struct {
                                       the survivors are compacted first (thresholded inputs) */
     int64_t n_regular;             /* apparent pairs whose cofacet vertex lies above every vertex of s (sorted by
                                       one stable partition); the other n_apparent - n_regular are sorted in full */
+    int64_t n_reduce_serial;       /* non-apparent columns whose reduction needed another non-apparent column (or did not
+                                      fit a warp's working column): taken by the CTA-level lock-free reduction */
+    int64_t n_reduce_displaced;    /* times a column took a pivot row from a later column that had claimed it first */
+    int64_t reduce_arena_bytes;    /* device bytes of reduced columns and working buffers the reduction used */
     int32_t key_bits;              /* bits of the diameter rank inside a packed record */
     int32_t index_bits;            /* bits of the vertex word inside a packed column record */
     int32_t sort_passes;           /* radix passes run by the filtration sort */
@@ -96,22 +100,38 @@ typedef struct {
     float stage1_ms;         /* whole stage 1 as enqueued (including memsets, scalar read-back) */
     float stage2_ms;         /* whole stage 2 */
     float dim0_ms;           /* d == 0 only: edge sort is part of rips_init; this is the union-find kernel */
-    float reduce_device_ms;  /* NOT hot path: non-apparent columns reduced against the apparent ones on the device */
-    float reduce_host_ms;    /* NOT hot path: serial remainder (conflicts between non-apparent columns) on the host */
-    float reduce_xfer_ms;    /* NOT hot path: D2H/H2D copies around the host reduction */
+    float reduce_device_ms;  /* NOT hot path: the reduction of the non-apparent columns, all of it on the device (host clock
+                                around the kernels, their set-up and the read-back of the counters) */
+    float reduce_host_ms;    /* always 0: no part of the reduction runs on the host (kept for the round-1 layout) */
+    float reduce_xfer_ms;    /* NOT hot path: D2H copy of the bars */
 } rips_timings_t;
 
-/* Estimate (an upper bound up to allocator rounding), in bytes, of the device memory rips_compute holds for (n, dim_max) with no
- * threshold (a threshold only lowers it).  RIPS_EOVERFLOW if the sizes do not fit. */
+/* Upper bound, in bytes, of the workspace rips_init + rips_compute + every accessor of dimensions 0..dim_max use for n
+ * points with no threshold (a threshold only lowers the use), including 256 MB / 64 bytes per candidate of arena for
+ * the reduced columns of rips_reduce.  What it does NOT bound: the reduced columns of inputs on which they fill in
+ * ("difficult datasets"; e.g. a 400-point random matrix needs 42 GB in dimension 1) and the stages at
+ * d = dim_max + 1.  RIPS_EOVERFLOW if the sizes do not fit. */
 int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes);
+
+/* After a call on this thread returned RIPS_ENOMEM: the workspace size with which that request would have fitted (the
+ * size in use, fragmentation included, plus the request), 0 if unknown. */
+int64_t rips_last_required_bytes(void);
 
 /* Create a context.  dist_lower: n(n-1)/2 fp32, HOST or DEVICE pointer (detected), layout above.
  * dim_max in [0,4]: H_0..H_dim_max.  threshold: keep simplices of diameter <= threshold
  * (inclusive); +INFINITY = full complex; the library never substitutes the
- * enclosing radius on its own.  stream: a cudaStream_t cast to void*, NULL = the
- * default stream.  Validates the matrix (RIPS_EINVAL on NaN, negative or infinite entries), copies
- * it, ranks the distinct edge values on the device and builds the binomial table.  */
-int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* stream);
+ * enclosing radius on its own.
+ * workspace_dev / workspace_bytes: DEVICE memory (256-byte aligned) every device array of the context is carved
+ * from; it stays the caller's, must outlive the context, and nothing in the library allocates or frees device
+ * memory between rips_init and rips_free.  A request that does not fit returns RIPS_ENOMEM (the size that would
+ * have fitted: rips_last_required_bytes); the context stays usable.  workspace_dev = NULL: rips_init allocates the
+ * workspace itself (cudaMalloc, sized for this input and threshold; freed by rips_free) and adds to it only if a
+ * computation needs more than was foreseen.
+ * stream: a cudaStream_t cast to void*, NULL = the default stream.  Validates the matrix (RIPS_EINVAL on NaN,
+ * negative or infinite entries), copies it, ranks the distinct edge values on the device and builds the binomial
+ * table.  */
+int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* workspace_dev,
+              int64_t workspace_bytes, void* stream);
 
 /* Dimension 0 .. dim_max, all stages: dim 0, then per d: stage 1, stage 2, reduction. */
 int rips_compute(rips_ctx* ctx);
@@ -156,8 +176,10 @@ int rips_pivot_lookup(rips_ctx* ctx, int d, const uint64_t* t_query_dev, int64_t
 int rips_stats(rips_ctx* ctx, int d, rips_stats_t* out);
 int rips_timings(rips_ctx* ctx, int d, rips_timings_t* out);
 
-/* Device bytes currently held by the context. */
+/* Size of the context's workspace in bytes (constant between rips_init and rips_free with a caller's workspace). */
 int rips_device_bytes(rips_ctx* ctx, int64_t* bytes);
+/* Bytes of the workspace handed out right now, and the largest value that has had (peak may be NULL). */
+int rips_workspace_in_use(rips_ctx* ctx, int64_t* bytes, int64_t* peak);
 /* Number of kernels this context has launched so far. */
 int rips_kernel_launches(rips_ctx* ctx, int64_t* launches);
 

@@ -2,7 +2,7 @@
 
     python -m paper_2003_07989_b200.build [--force] [--verbose]
 
-The sources are csrc/*.cu (hand-written CUDA) and csrc/reduce_host.cpp; the only public header is
+The sources are csrc/*.cu (hand-written CUDA); the only public header is
 include/rips.h.  The .so is git-ignored but travels to the GPU box with the tree.
 """
 from __future__ import annotations
@@ -15,8 +15,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librips_b200.so")
-SOURCES = ["rips.cu", "radix_sort.cu", "stage1.cu", "stage2.cu", "dim0.cu", "init.cu", "reduce.cu", "reduce_host.cpp"]
-HEADERS = ["common.cuh", "kernels.cuh", "apparent.cuh", "radix_sort.cuh", "reduce_host.h", os.path.join("..", "..", "include", "rips.h")]
+SOURCES = ["rips.cu", "radix_sort.cu", "stage1.cu", "stage2.cu", "dim0.cu", "init.cu", "reduce.cu"]
+HEADERS = ["common.cuh", "kernels.cuh", "apparent.cuh", "radix_sort.cuh", os.path.join("..", "..", "include", "rips.h")]
 
 
 def nvcc() -> str:

@@ -115,7 +115,15 @@ cudaError_t launch_pivot_lookup(int M, const PairLayers& L, BinomTable bt, int n
                                 i64 n2, const u64* query, i64 m, i64* s_out, cudaStream_t st);
 
 // ------------------------------------------------------------------ reduce.cu (not the hot path)
-struct PreReduceParams {
+// Reference to a reduced column in the arena: bit 63 = sorted, bits 62..27 = offset (entries), bits 26..0 = length.
+#define RD_REF(off, len, sorted) (((u64)(sorted) << 63) | ((u64)(off) << 27) | (u64)(len))
+#define RD_REF_OFF(r) (((r) >> 27) & ((1ull << 36) - 1ull))
+#define RD_REF_LEN(r) ((r) & ((1ull << 27) - 1ull))
+#define RD_REF_SORTED(r) ((r) >> 63)
+enum { RDC_ARENA_TOP = 0, RDC_ADDS = 1, RDC_TODO = 2, RDC_TICKET = 3, RDC_STEALS = 4, RDC_PIVOTS = 5, RDC_NBARS = 6, RDC_NESS = 7, RDC_DBG = 8, RDC_COUNT = 14 };
+enum { RD_ERR_ARENA = 1, RD_ERR_SORTCAP = 2, RD_ERR_PROTOCOL = 4, RD_ERR_STUCK = 8 };
+
+struct ReduceParams {
     const u64* cols;      // non-apparent column records, coboundary order
     i64 ncols;
     const void* Kf;
@@ -123,9 +131,30 @@ struct PreReduceParams {
     BinomTable bt;
     int vbits, tbits;
     u32 thr_key;          // cofacets with key < thr_key are above the threshold
-    PairLayers layers;    // apparent pairs of this dimension
-    u32 max_additions;    // columns needing more are left to the host
-    u64* pivot_out;       // per column: 0 = reduced to zero, ~0 = left to the host, else (key << tbits | cidx(t)) + 1
-    u32* adds_out;        // per column: additions performed
+    PairLayers layers;    // apparent pairs of this dimension (first layer of the pair store)
+    u64* piv;             // [ncols] 0 = zero column, ~0 = not reduced yet, else the pivot entry ((key << tbits | cidx(t)) + 1)
+    u64* colref;          // [ncols] RD_REF of the column's published reduced column
+    unsigned char* todo;  // [ncols] 1 = reduce_kernel has to take the column
+    u64* ht_keys;         // second layer of the pair store: open addressing, ~0 = empty
+    u32* ht_vals;         // owning column, 0xffffffff = none
+    u32 ht_mask;
+    u64* arena;           // reduced columns and working buffers
+    u64 arena_cap;        // entries
+    int sort_cap;         // entries a CTA can sort in shared memory (>= n, >= 2048, a power of two)
+    int workers;          // CTAs of reduce_kernel
+    u64* counters;        // RDC_*, zeroed
+    u32* error;           // RD_ERR_* flags, zeroed
 };
-cudaError_t launch_prereduce(int M, int kf_u16, const PreReduceParams& p, cudaStream_t st);
+size_t reduce_smem_bytes(int sort_cap);
+int reduce_sort_cap(int n);
+int reduce_workers(int sms, int sort_cap);
+// prereduce_kernel, claim_kernel, worklist_kernel, reduce_kernel: afterwards piv[] holds every column's pivot
+cudaError_t launch_reduce(int M, int kf_u16, const ReduceParams& p, int sms, cudaStream_t st);
+// rec[j] = (cidx(t) << jbits) | j (all ones for a zero column); counters[RDC_PIVOTS] += columns with a pivot
+cudaError_t launch_pivot_records(const ReduceParams& p, int jbits, u64* rec, cudaStream_t st);
+// rec sorted by t -> t_out[i], s_out[i] = cidx of the column (Eq. 2)
+cudaError_t launch_pivot_arrays(int M, const ReduceParams& p, int jbits, const u64* rec, i64 n_piv, u64* t_out, u64* s_out,
+                                cudaStream_t st);
+// bars (birth, death) in column order, zero-length ones dropped, +inf for zero columns; counts to n_bars / n_essential
+cudaError_t launch_bars(const ReduceParams& p, int lowbits, const float* values, float* bars, u64* n_bars, u64* n_essential,
+                        cudaStream_t st);

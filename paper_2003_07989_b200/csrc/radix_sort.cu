@@ -5,7 +5,6 @@
 // in increasing combinatorial index leave each pass in increasing index within equal digits: the
 // index bits never have to be sorted.
 #include "radix_sort.cuh"
-#include <cstdlib>
 
 namespace {
 
@@ -101,7 +100,6 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 // look-back at once, scan over the bins; (4) records placed in tile-sorted order in shared memory;
 // (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
-template <bool MATCH, bool EARLY>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
                      const u64* __restrict__ global_base, u64* status, u32* ticket, int pf_dist)
@@ -113,16 +111,14 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     u64* goff = stage + SORT_TILE;                                        // [MAX_BINS]
     u32* whist = reinterpret_cast<u32*>(goff + RIPS_SORT_MAX_BINS);       // [SORT_WARPS][MAX_BINS]
     u32* bin_start = whist + SORT_WARPS * RIPS_SORT_MAX_BINS;             // [MAX_BINS]
-    u32* thist = bin_start + RIPS_SORT_MAX_BINS;                          // [MAX_BINS] (EARLY only)
     __shared__ u32 s_tile;
     __shared__ u32 s_wsum[8];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = ticket ? atomicAdd(ticket, 1u) : blockIdx.x;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u); // tiles numbered in the order they start: every predecessor is resident or done
     u32* wh = whist + warp * RIPS_SORT_MAX_BINS;
 #pragma unroll
     for (int i = lane; i < RIPS_SORT_MAX_BINS; i += 32) wh[i] = 0;
-    if (EARLY && tid < RIPS_SORT_MAX_BINS) thist[tid] = 0;
     __syncthreads();
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
@@ -154,27 +150,6 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
         }
     }
 
-    // ---- (1b) EARLY: the tile's digit counts by plain shared atomics, published for the look-back
-    // before the ranking, so that the tiles behind this one never wait for its ranking (the ranking
-    // is the longest phase of a tile; the look-back below then finds every predecessor published).
-    if (EARLY) {
-#pragma unroll
-        for (int i = 0; i < SORT_IPT; ++i) {
-            const u32 d = (u32)(key[i] >> shift) & mask;
-            const u32 d0 = __shfl_sync(RIPS_FULL_MASK, d, 0);
-            if (__all_sync(RIPS_FULL_MASK, d == d0)) { // skewed digits: one add per warp instead of 32 serialised ones
-                if (lane == 0) atomicAdd(&thist[d0], 32u);
-            } else {
-                atomicAdd(&thist[d], 1u);
-            }
-        }
-        __syncthreads();
-        if (tid < nbins) {
-            const u32 c = thist[tid] - ((tid == nbins - 1) ? (u32)(SORT_TILE - count) : 0u);
-            st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)c);
-        }
-    }
-
     // ---- (2) rank inside the warp.  Three pipelined phases instead of one latency chain per record:
     // all MATCHes, then one shared-memory atomic per digit group and round (the rounds of a warp
     // reach its histogram in program order, so the value returned is the count of the earlier
@@ -186,23 +161,9 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
 #pragma unroll
         for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
             const u32 d = (u32)(key[i] >> shift) & mask;
-            if (MATCH) {
-                // one MATCH per record: ~2 cycles per DISTINCT digit in the warp (measured), so only for
-                // skewed digits (the partition of the pairs by cofacet vertex)
-                rank[i] = __match_any_sync(RIPS_FULL_MASK, d);
-            } else {
-                // one ballot per digit bit: flat cost, cheaper than MATCH once a warp holds many digits
-                u32 peers = RIPS_FULL_MASK;
-#pragma unroll
-                for (int b = 0; b < 8; ++b) {
-                    if (b < bits) {
-                        const bool bit = (d >> b) & 1u;
-                        const u32 bal = __ballot_sync(RIPS_FULL_MASK, bit);
-                        peers &= bit ? bal : ~bal;
-                    }
-                }
-                rank[i] = peers;
-            }
+            // one MATCH per record (~2 cycles per distinct digit in the warp); one ballot per digit bit was
+            // measured slower at every pass of this workload
+            rank[i] = __match_any_sync(RIPS_FULL_MASK, d);
         }
         u32 old[SORT_RANK_BATCH];
 #pragma unroll
@@ -233,8 +194,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
                 run += c;
             }
             my_count = (tid == nbins - 1) ? run - (u32)n_pad : run;
-            if (!EARLY)
-                st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
+            st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
         }
         // block scan of `run` over the first MAX_BINS threads (8 warps)
         u32 incl = run;
@@ -326,7 +286,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
 size_t pass_smem_bytes(int)
 {
     const size_t nb = RIPS_SORT_MAX_BINS;
-    return (size_t)SORT_TILE * 8 + nb * 8 + (size_t)SORT_WARPS * nb * 4 + nb * 4 + nb * 4;
+    return (size_t)SORT_TILE * 8 + nb * 8 + (size_t)SORT_WARPS * nb * 4 + nb * 4;
 }
 
 struct ScratchLayout {
@@ -381,30 +341,25 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
                      SortTimes* times, i64* launches, bool hist_ready, bool skewed_digits)
 {
     *result = a;
+    int sms = 148;
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     if (times && times->enabled) cudaEventRecord(times->ev[0], stream);
     if (n <= 1) {
         if (times && times->enabled) { cudaEventRecord(times->ev[1], stream); cudaEventRecord(times->ev[2], stream); }
         return cudaSuccess;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaSuccess;
-        const void* fns[4] = {(const void*)onesweep_pass_kernel<true, false>, (const void*)onesweep_pass_kernel<false, false>,
-                              (const void*)onesweep_pass_kernel<true, true>, (const void*)onesweep_pass_kernel<false, true>};
-        for (int f = 0; f < 4; ++f) {
-            e = cudaFuncSetAttribute(fns[f], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
-            if (e != cudaSuccess) return e;
-        }
+    {   // per call (cheap) rather than once per process: the attribute is per device
+        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
+        if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(sort_histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 4);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
-    static const int force_rank = getenv("RIPS_SORT_RANK") ? atoi(getenv("RIPS_SORT_RANK")) : 1; // tuning: 0 ballots, 1 match
-    static const int early = getenv("RIPS_SORT_EARLY") ? atoi(getenv("RIPS_SORT_EARLY")) : 0; // tuning: 0 publish after the ranking
-    static const int use_ticket = getenv("RIPS_SORT_TICKET") ? atoi(getenv("RIPS_SORT_TICKET")) : 1; // measurement only: 0 = tile from blockIdx.x
-    static const int pf_dist = getenv("RIPS_SORT_PF") ? atoi(getenv("RIPS_SORT_PF")) : 148; // tuning: tiles ahead, 0 = off
-    if (force_rank >= 0) skewed_digits = force_rank != 0;
+    const int pf_dist = sms; // tiles ahead of the L2 prefetch: one wave (swept 0 .. 12 waves in round 1)
+    (void)skewed_digits;
     ScratchLayout L = scratch_layout(n, plan);
     unsigned char* sc = (unsigned char*)scratch;
     u64* hist = (u64*)(sc + L.hist_off);
@@ -421,7 +376,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     {
         i64 chunk = (i64)HIST_THREADS * HIST_IPT;
         i64 blocks = (n + chunk - 1) / chunk;
-        if (blocks > 148 * 4) blocks = 148 * 4;
+        if (blocks > (i64)sms * 4) blocks = (i64)sms * 4;
         if (!hist_ready) {
             sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, pd, hist);
             if (launches) *launches += 1;
@@ -436,12 +391,8 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         size_t status_bytes = (size_t)tiles * ((size_t)1 << plan.bits[p]) * 8;
         e = cudaMemsetAsync(status, 0, status_bytes, stream);
         if (e != cudaSuccess) return e;
-#define RIPS_SORT_LAUNCH(M, E)                                                                                      \
-    onesweep_pass_kernel<M, E><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(          \
-        src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, use_ticket ? ticket + p : (u32*)nullptr, pf_dist)
-        if (skewed_digits) { if (early) RIPS_SORT_LAUNCH(true, true); else RIPS_SORT_LAUNCH(true, false); }
-        else               { if (early) RIPS_SORT_LAUNCH(false, true); else RIPS_SORT_LAUNCH(false, false); }
-#undef RIPS_SORT_LAUNCH
+        onesweep_pass_kernel<<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
+            src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist);
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }

@@ -17,7 +17,6 @@
 
 #include "kernels.cuh"
 #include "radix_sort.cuh"
-#include "reduce_host.h"
 
 namespace {
 
@@ -39,11 +38,95 @@ int cuda_fail(cudaError_t e, const char* what)
         if (r__ != RIPS_OK) return r__; \
     } while (0)
 
-// A device buffer that is reused while large enough.
+// A device buffer that is reused while large enough; carved from the context's workspace (Pool).
 struct DevBuf {
     void* p = nullptr;
     size_t cap = 0;
 };
+
+// The workspace: one device allocation (the caller's, or the library's own made by rips_init) managed on the host
+// as a list of blocks, first fit, 256-byte granules.  Nothing between rips_init and rips_free calls cudaMalloc /
+// cudaFree, unless the library owns the workspace AND a computation needs more than rips_workspace_bytes foresaw
+// (the reduced columns of a difficult input, views of thresholded inputs): then a further chunk is added.
+struct Pool {
+    struct Chunk {
+        unsigned char* base = nullptr;
+        size_t size = 0;
+        bool owned = false;
+        struct Blk { size_t off, size; bool used; };
+        std::vector<Blk> blks;
+    };
+    std::vector<Chunk> chunks;
+    bool may_grow = false;
+    size_t in_use = 0, peak = 0;
+
+    static size_t round(size_t b) { return (b + 255) & ~(size_t)255; }
+    void add_chunk(void* base, size_t size, bool owned)
+    {
+        Chunk ch;
+        ch.base = (unsigned char*)base;
+        ch.size = size & ~(size_t)255;
+        ch.owned = owned;
+        ch.blks.push_back({0, ch.size, false});
+        chunks.push_back(std::move(ch));
+    }
+    void* alloc(size_t bytes)
+    {
+        bytes = round(bytes ? bytes : 1);
+        for (Chunk& ch : chunks)
+            for (size_t i = 0; i < ch.blks.size(); ++i) {
+                Chunk::Blk& b = ch.blks[i];
+                if (b.used || b.size < bytes) continue;
+                if (b.size > bytes) {
+                    Chunk::Blk rest{b.off + bytes, b.size - bytes, false};
+                    b.size = bytes;
+                    b.used = true;
+                    const size_t off = b.off;
+                    ch.blks.insert(ch.blks.begin() + (long)i + 1, rest);
+                    in_use += bytes;
+                    peak = std::max(peak, in_use);
+                    return ch.base + off;
+                }
+                b.used = true;
+                in_use += bytes;
+                peak = std::max(peak, in_use);
+                return ch.base + b.off;
+            }
+        return nullptr;
+    }
+    void free(void* p)
+    {
+        if (!p) return;
+        for (Chunk& ch : chunks) {
+            if ((unsigned char*)p < ch.base || (unsigned char*)p >= ch.base + ch.size) continue;
+            const size_t off = (size_t)((unsigned char*)p - ch.base);
+            for (size_t i = 0; i < ch.blks.size(); ++i) {
+                if (ch.blks[i].off != off || !ch.blks[i].used) continue;
+                ch.blks[i].used = false;
+                in_use -= ch.blks[i].size;
+                if (i + 1 < ch.blks.size() && !ch.blks[i + 1].used) { ch.blks[i].size += ch.blks[i + 1].size; ch.blks.erase(ch.blks.begin() + (long)i + 1); }
+                if (i > 0 && !ch.blks[i - 1].used) { ch.blks[i - 1].size += ch.blks[i].size; ch.blks.erase(ch.blks.begin() + (long)i); }
+                return;
+            }
+        }
+    }
+    size_t largest_free() const
+    {
+        size_t m = 0;
+        for (const Chunk& ch : chunks)
+            for (const Chunk::Blk& b : ch.blks)
+                if (!b.used) m = std::max(m, b.size);
+        return m;
+    }
+    size_t total() const
+    {
+        size_t t = 0;
+        for (const Chunk& ch : chunks) t += ch.size;
+        return t;
+    }
+};
+
+thread_local int64_t g_required_bytes = 0;
 
 enum Ev {
     EV_S1_BEGIN, EV_S1_BITMAP, EV_S1_ENUM, EV_S1_SORTBEG, EV_S1_HIST, EV_S1_SORT, EV_S1_END,
@@ -59,9 +142,11 @@ struct DimState {
     int compact = 0;
     // stage 1: column records (sorted), pair slots (unsorted until stage 2), the two small lists
     bool have_s1 = false;
-    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch, pre_piv, pre_adds;
+    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch;
+    DevBuf rd_piv, rd_colref, rd_todo, rd_htk, rd_htv, rd_arena, rd_cnt, rd_rec, rd_rec2, rd_bars; // reduction
     u64* cols = nullptr; // sorted packed column records (points into colsA or colsB)
     i64 len = 0;         // columns
+    i64 exact_kept = -1; // compact mode: columns counted by the first run of this dimension (a constant of the context)
     i64 slots = 0;       // records in the column / pair arrays (len in compact mode, else C(n,d+1) with sentinels)
     SortPlan pair_plan;
     bool pair_fused = false, pairs_fresh = false;
@@ -99,16 +184,15 @@ struct rips_ctx {
     int kmax = 0; // binomial table holds C(v,k), k <= kmax
     std::vector<u64> h_binom;
     std::vector<float> h_values;
-    std::vector<u32> h_K; // host copy of the key matrix, made on first use by the reduction
     float* d_dist = nullptr;
     u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
     u32* d_K = nullptr;
     void* d_Kf = nullptr;  // full symmetric matrix of key+1 (common.cuh)
     int kf_u16 = 0, kf_pitch = 1, vbits = 1;
-    int fast_visits = 0; // tuning override (RIPS_FAST_VISITS), 0 = per-dimension default
+    int sms = 148;       // multiprocessors of the device
     float* d_values = nullptr;
     u64* d_binom = nullptr;
-    u64* d_counters = nullptr; // 8 u64 scratch counters
+    u64* d_counters = nullptr; // 16 u64 scratch counters
     u32* d_tickets = nullptr;  // 8 u32
     u64* h_counters = nullptr; // pinned
     u32 n_distinct = 0, thr_key = 0;
@@ -117,7 +201,9 @@ struct rips_ctx {
     // dim 0
     DevBuf d0_pairs, d0_death, d0_uf;
     std::vector<DimState> dims; // index d, 0 .. dim_max+1
-    i64 dev_bytes = 0, launches = 0;
+    Pool pool;
+    DevBuf b_dist, b_edges, b_K, b_Kf, b_values, b_binom, b_counters, b_tickets, b_init_tmp, b_init_status;
+    i64 launches = 0;
     BinomTable bt() const { return BinomTable{d_binom, (int)(n + 1)}; }
 };
 
@@ -127,21 +213,33 @@ int ensure(rips_ctx* c, DevBuf& b, size_t bytes)
 {
     if (bytes == 0) bytes = 16;
     if (b.cap >= bytes) return RIPS_OK;
-    if (b.p) { cudaFree(b.p); c->dev_bytes -= (i64)b.cap; b.p = nullptr; b.cap = 0; }
-    cudaError_t e = cudaMalloc(&b.p, bytes);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        g_last_error = "cudaMalloc of " + std::to_string(bytes) + " bytes failed: " + cudaGetErrorString(e);
-        b.p = nullptr;
-        return e == cudaErrorMemoryAllocation ? RIPS_ENOMEM : RIPS_ECUDA;
+    if (b.p) { c->pool.free(b.p); b.p = nullptr; b.cap = 0; }
+    void* q = c->pool.alloc(bytes);
+    if (!q && c->pool.may_grow) {
+        // the library owns the workspace and the estimate fell short: one more chunk
+        size_t chunk = std::max<size_t>(Pool::round(bytes), (size_t)256 << 20);
+        void* base = nullptr;
+        cudaError_t e = cudaMalloc(&base, chunk);
+        if (e != cudaSuccess) { cudaGetLastError(); chunk = Pool::round(bytes); e = cudaMalloc(&base, chunk); }
+        if (e == cudaSuccess) {
+            c->pool.add_chunk(base, chunk, true);
+            q = c->pool.alloc(bytes);
+        } else
+            cudaGetLastError();
     }
-    b.cap = bytes;
-    c->dev_bytes += (i64)bytes;
+    if (!q) {
+        g_required_bytes = (int64_t)(c->pool.total() - c->pool.largest_free() + Pool::round(bytes));
+        g_last_error = "workspace too small: " + std::to_string(bytes) + " more bytes needed with " + std::to_string(c->pool.in_use) + " of " +
+                       std::to_string(c->pool.total()) + " in use (rips_last_required_bytes: " + std::to_string(g_required_bytes) + ")";
+        return RIPS_ENOMEM;
+    }
+    b.p = q;
+    b.cap = Pool::round(bytes);
     return RIPS_OK;
 }
 void release(rips_ctx* c, DevBuf& b)
 {
-    if (b.p) { cudaFree(b.p); c->dev_bytes -= (i64)b.cap; }
+    if (b.p) c->pool.free(b.p);
     b.p = nullptr;
     b.cap = 0;
 }
@@ -308,6 +406,9 @@ int run_stage1(rips_ctx* c, int d)
         keep_stats.n_essential = s.stats.n_essential;
         keep_stats.n_additions = s.stats.n_additions;
         keep_stats.n_bars = s.stats.n_bars;
+        keep_stats.n_reduce_serial = s.stats.n_reduce_serial;
+        keep_stats.n_reduce_displaced = s.stats.n_reduce_displaced;
+        keep_stats.reduce_arena_bytes = s.stats.reduce_arena_bytes;
     }
     s.stats = keep_stats;
     s.stats.n_candidates = (i64)s.total;
@@ -368,7 +469,7 @@ int run_stage1(rips_ctx* c, int d)
     p.clear = cs;
     p.compact = s.compact;
     p.count_only = 0;
-    p.fast_visits = c->fast_visits > 0 ? c->fast_visits : 16; // swept at cfg 2 (4..32): flat above 12
+    p.fast_visits = 16; // swept at cfg 2 (4..32): flat above 12
     p.cols_out = p.pairs_out = p.irr_out = p.non_out = nullptr;
     p.irr_cap = p.non_cap = 0;
     p.status = nullptr;
@@ -379,9 +480,8 @@ int run_stage1(rips_ctx* c, int d)
 
     u64 cap = s.total; // slots of the two record arrays
     if (s.compact) {
-        size_t free_b = 0, total_b = 0;
-        cudaMemGetInfo(&free_b, &total_b);
-        if (s.total * 8 > free_b / 16 && s.colsA.cap < s.total * 8) { // count first, then allocate exactly
+        if (s.exact_kept >= 0) cap = (u64)s.exact_kept; // the count is a constant of the context
+        else { // first run of this dimension: count, then size the arrays exactly
             CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
             CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
             p.count_only = 1;
@@ -391,6 +491,7 @@ int run_stage1(rips_ctx* c, int d)
             CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
             cap = c->h_counters[S1C_KEPT];
+            s.exact_kept = (i64)cap;
         }
         RC(ensure(c, s.s1_status, (size_t)tiles * 8));
         p.status = (u64*)s.s1_status.p;
@@ -404,9 +505,8 @@ int run_stage1(rips_ctx* c, int d)
     s.pair_plan = sort_make_plan(s.tbits, s.tbits + pvbits);
     RC(ensure(c, c->sort_scratch, sort_scratch_bytes((i64)cap, plan)));
     RC(ensure(c, s.pair_scratch, sort_scratch_bytes((i64)cap, s.pair_plan)));
-    static const int nofuse = getenv("RIPS_NO_FUSED_HIST") ? atoi(getenv("RIPS_NO_FUSED_HIST")) : 0; // tuning: bit 0 columns, bit 1 pairs
-    const bool fused = plan.npasses <= 3 && !(nofuse & 1);           // S1_MAX_FUSED digits
-    s.pair_fused = s.pair_plan.npasses <= 2 && !(nofuse & 2);        // S1_MAX_FUSED_P digits
+    const bool fused = plan.npasses <= 3;           // S1_MAX_FUSED digits
+    s.pair_fused = s.pair_plan.npasses <= 2;        // S1_MAX_FUSED_P digits
     // provisioned for (d+1)/n of the columns to hold the top vertices (those pairs are irregular) and as many
     // non-apparent ones; a run that needs more is repeated once with the exact sizes
     u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 8));
@@ -576,108 +676,134 @@ int run_reduce(rips_ctx* c, int d)
     invalidate_views(s, false, false, false, true);
     s.bars.clear();
     s.tim.reduce_host_ms = s.tim.reduce_xfer_ms = s.tim.reduce_device_ms = 0.f;
-    HostReduceOut out;
+    i64 n_piv = 0, n_ess = 0, n_adds = 0;
     if (s.n_non > 0) {
-        // ---- device: every non-apparent column reduced against the apparent columns (reduce.cu)
-        std::vector<u64> h_pre((size_t)s.n_non);
-        std::vector<u32> h_adds((size_t)s.n_non);
-        {
-            double td = now_ms();
-            RC(ensure(c, s.pre_piv, (size_t)s.n_non * 8));
-            RC(ensure(c, s.pre_adds, (size_t)s.n_non * 4));
-            PreReduceParams pp;
-            pp.cols = s.non;
-            pp.ncols = s.n_non;
-            pp.Kf = c->d_Kf;
-            pp.pitch = c->kf_pitch;
-            pp.n = (int)c->n;
-            pp.bt = c->bt();
-            pp.vbits = c->vbits;
-            pp.tbits = s.tbits;
-            pp.thr_key = c->thr_key;
-            pp.layers = layers_of(s);
-            pp.max_additions = 64;
-            pp.pivot_out = (u64*)s.pre_piv.p;
-            pp.adds_out = (u32*)s.pre_adds.p;
-            CU(launch_prereduce(s.M, c->kf_u16, pp, c->stream));
-            c->launches += 1;
-            CU(cudaMemcpyAsync(h_pre.data(), s.pre_piv.p, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost, c->stream));
-            CU(cudaMemcpyAsync(h_adds.data(), s.pre_adds.p, (size_t)s.n_non * 4, cudaMemcpyDeviceToHost, c->stream));
+        const double t0 = now_ms();
+        const i64 nn = s.n_non;
+        const int jbits = bits_for((u64)(nn - 1));
+        if (s.tbits + jbits > 64) { g_last_error = "rips_reduce: (row, column) records do not fit 64 bits"; return RIPS_EOVERFLOW; }
+        u32 ht_cap = 1024;
+        while ((u64)ht_cap < 2ull * (u64)nn) ht_cap <<= 1;
+        const int sort_cap = reduce_sort_cap((int)c->n);
+        if (reduce_smem_bytes(sort_cap) > 200u * 1024u) {
+            g_last_error = "rips_reduce: more points than a CTA can sort the coboundary of in shared memory (n <= 16384)";
+            return RIPS_EOVERFLOW;
+        }
+        const int workers = reduce_workers(c->sms, sort_cap);
+        RC(ensure(c, s.rd_piv, (size_t)nn * 8));
+        RC(ensure(c, s.rd_colref, (size_t)nn * 8));
+        RC(ensure(c, s.rd_todo, (size_t)nn));
+        RC(ensure(c, s.rd_htk, (size_t)ht_cap * 8));
+        RC(ensure(c, s.rd_htv, (size_t)ht_cap * 4));
+        RC(ensure(c, s.rd_cnt, (size_t)(RDC_COUNT + 1) * 8));
+        RC(ensure(c, s.rd_rec, (size_t)nn * 8));
+        RC(ensure(c, s.rd_rec2, (size_t)nn * 8));
+        RC(ensure(c, s.rd_bars, (size_t)nn * 8));
+        // the arena holds every reduced column and the working buffers; how much the columns fill in depends on
+        // the input, so a run that exhausts it is repeated with a larger one
+        // (library-owned workspace: a further chunk; caller's workspace: RIPS_ENOMEM with the size the next attempt
+        // would have asked for).  First attempt: the largest free block of the workspace, at most 64 bytes per slot.
+        size_t arena_bytes = s.rd_arena.cap;
+        if (!arena_bytes) {
+            const size_t want = std::max<size_t>((size_t)256 << 20, (size_t)s.slots * 64);
+            const size_t have = c->pool.largest_free();
+            arena_bytes = std::min(want, have);
+            if (arena_bytes < ((size_t)16 << 20)) arena_bytes = want;
+        }
+        ReduceParams p;
+        for (int attempt = 0;; ++attempt) {
+            size_t limit = ~(size_t)0;
+            if (c->pool.may_grow) {
+                size_t free_b = 0, total_b = 0;
+                cudaMemGetInfo(&free_b, &total_b);
+                limit = s.rd_arena.cap + c->pool.largest_free() + (size_t)((double)free_b * 0.9);
+                if (arena_bytes > limit) arena_bytes = limit;
+            }
+            RC(ensure(c, s.rd_arena, arena_bytes));
+            p.cols = s.non;
+            p.ncols = nn;
+            p.Kf = c->d_Kf;
+            p.pitch = c->kf_pitch;
+            p.n = (int)c->n;
+            p.bt = c->bt();
+            p.vbits = c->vbits;
+            p.tbits = s.tbits;
+            p.thr_key = c->thr_key;
+            p.layers = layers_of(s);
+            p.piv = (u64*)s.rd_piv.p;
+            p.colref = (u64*)s.rd_colref.p;
+            p.todo = (unsigned char*)s.rd_todo.p;
+            p.ht_keys = (u64*)s.rd_htk.p;
+            p.ht_vals = (u32*)s.rd_htv.p;
+            p.ht_mask = ht_cap - 1;
+            p.arena = (u64*)s.rd_arena.p;
+            p.arena_cap = (u64)(s.rd_arena.cap / 8);
+            p.sort_cap = sort_cap;
+            p.workers = workers;
+            p.counters = (u64*)s.rd_cnt.p;
+            p.error = (u32*)((u64*)s.rd_cnt.p + RDC_COUNT);
+            CU(cudaMemsetAsync(s.rd_cnt.p, 0, (size_t)(RDC_COUNT + 1) * 8, c->stream));
+            CU(cudaMemsetAsync(s.rd_colref.p, 0, (size_t)nn * 8, c->stream));
+            CU(cudaMemsetAsync(s.rd_htk.p, 0xff, (size_t)ht_cap * 8, c->stream));
+            CU(cudaMemsetAsync(s.rd_htv.p, 0xff, (size_t)ht_cap * 4, c->stream));
+            CU(launch_reduce(s.M, c->kf_u16, p, c->sms, c->stream));
+            c->launches += 4;
+            CU(cudaMemcpyAsync(c->h_counters, s.rd_cnt.p, (size_t)(RDC_COUNT + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
-            s.tim.reduce_device_ms = (float)(now_ms() - td);
-            for (u32 a : h_adds) out.additions += a;
-        }
-        double t0 = now_ms();
-        if (c->h_K.empty() && c->E) {
-            c->h_K.resize((size_t)c->E);
-            CU(cudaMemcpy(c->h_K.data(), c->d_K, (size_t)c->E * 4, cudaMemcpyDeviceToHost));
-        }
-        std::vector<u64> h_non((size_t)s.n_non);
-        CU(cudaMemcpy(h_non.data(), s.non, (size_t)s.n_non * 8, cudaMemcpyDeviceToHost));
-        {   // vertex-packed column records -> (key << cbits) | cidx for the host reduction (Eq. 2)
-            const u64 vmask = (1ull << c->vbits) - 1ull;
-            for (u64& r : h_non) {
-                u64 cidx = 0;
-                for (int j = 0; j < s.M; ++j) cidx += hbinom(c, (i64)((r >> (j * c->vbits)) & vmask), j + 1);
-                r = ((r >> s.lowbits) << s.cbits) | cidx;
+            const u32 err = (u32)c->h_counters[RDC_COUNT];
+            if (!err) break;
+            if ((err & RD_ERR_ARENA) && attempt < 4 && arena_bytes < limit) { arena_bytes *= 8; continue; }
+            if (err & RD_ERR_ARENA) {
+                g_last_error = "rips_reduce: the reduced columns do not fit the device memory left (" + std::to_string(arena_bytes) + " bytes of arena)";
+                return RIPS_ENOMEM;
             }
+            g_last_error = (err & RD_ERR_SORTCAP) ? "rips_reduce: a coboundary exceeds the CTA's sort capacity"
+                                                  : "rips_reduce: internal error " + std::to_string(err) + " at column " + std::to_string(c->h_counters[RDC_DBG]) +
+                                                        " length " + std::to_string(c->h_counters[RDC_DBG + 1]) + " pivot " + std::to_string(c->h_counters[RDC_DBG + 2]) +
+                                                        " work item " + std::to_string(c->h_counters[RDC_DBG + 3]);
+            return RIPS_ECUDA;
         }
-        double t1 = now_ms();
-        HostReduceIn in;
-        in.n = (int)c->n;
-        in.d = d;
-        in.K = c->h_K.data();
-        in.binom = c->h_binom.data();
-        in.bstride = (int)(c->n + 1);
-        in.thr_key = c->thr_key;
-        in.n_keys = c->n_distinct;
-        in.cols = h_non.data();
-        in.ncols = s.n_non;
-        in.cbits = s.cbits;
-        in.tbits = s.tbits;
-        in.pre = h_pre.data();
-        host_reduce_columns(in, out);
-        double t2 = now_ms();
-        s.tim.reduce_host_ms = (float)(t2 - t1);
-        s.tim.reduce_xfer_ms = (float)(t1 - t0);
+#ifdef RIPS_REDUCE_PROFILE
+        fprintf(stderr, "reduce d=%d: cycles summed over CTAs: peek %llu apparent %llu coboundary+sort %llu add %llu other-add %llu\n", d,
+                (unsigned long long)c->h_counters[RDC_DBG], (unsigned long long)c->h_counters[RDC_DBG + 1], (unsigned long long)c->h_counters[RDC_DBG + 2],
+                (unsigned long long)c->h_counters[RDC_DBG + 3], (unsigned long long)c->h_counters[RDC_DBG + 4]);
+#endif
+        n_adds = (i64)c->h_counters[RDC_ADDS];
+        s.stats.n_reduce_serial = (i64)c->h_counters[RDC_TODO];
+        s.stats.n_reduce_displaced = (i64)c->h_counters[RDC_STEALS];
+        s.stats.reduce_arena_bytes = (i64)c->h_counters[RDC_ARENA_TOP] * 8;
+        // ---- second layer of the pair store as sorted arrays (t ascending), and the bars in column order
+        CU(launch_pivot_records(p, jbits, (u64*)s.rd_rec.p, c->stream));
+        SortPlan plan = sort_make_plan(jbits, jbits + s.tbits);
+        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(nn, plan)));
+        u64* sorted = nullptr;
+        CU(sort_u64((u64*)s.rd_rec.p, (u64*)s.rd_rec2.p, nn, plan, c->sort_scratch2.p, c->stream, &sorted, nullptr, &c->launches));
+        CU(launch_bars(p, s.lowbits, c->d_values, (float*)s.rd_bars.p, p.counters + RDC_NBARS, p.counters + RDC_NESS, c->stream));
+        c->launches += 2;
+        CU(cudaMemcpyAsync(c->h_counters, s.rd_cnt.p, (size_t)RDC_COUNT * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        n_piv = (i64)c->h_counters[RDC_PIVOTS];
+        n_ess = (i64)c->h_counters[RDC_NESS];
+        const i64 n_bars = (i64)c->h_counters[RDC_NBARS];
+        RC(ensure(c, s.red_t, (size_t)n_piv * 8));
+        RC(ensure(c, s.red_s, (size_t)n_piv * 8));
+        CU(launch_pivot_arrays(s.M, p, jbits, sorted, n_piv, (u64*)s.red_t.p, (u64*)s.red_s.p, c->stream));
+        c->launches += n_piv > 0;
+        const double t1 = now_ms();
+        s.bars.resize((size_t)n_bars * 2);
+        if (n_bars) CU(cudaMemcpyAsync(s.bars.data(), s.rd_bars.p, (size_t)n_bars * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        const double t2 = now_ms();
+        s.tim.reduce_device_ms = (float)(t1 - t0);
+        s.tim.reduce_xfer_ms = (float)(t2 - t1);
+    } else {
+        RC(ensure(c, s.red_t, 16));
+        RC(ensure(c, s.red_s, 16));
     }
-    // bars in column order of the birth simplex: merge the two lists by column position
-    {
-        size_t a = 0, b = 0;
-        while (a < out.piv_col.size() || b < out.ess_col.size()) {
-            bool take_piv = b >= out.ess_col.size() || (a < out.piv_col.size() && out.piv_col[a] < out.ess_col[b]);
-            if (take_piv) {
-                if (out.piv_key_s[a] != out.piv_key_t[a]) {
-                    s.bars.push_back(c->h_values[out.piv_key_s[a]]);
-                    s.bars.push_back(c->h_values[out.piv_key_t[a]]);
-                }
-                ++a;
-            } else {
-                s.bars.push_back(c->h_values[out.ess_key[b]]);
-                s.bars.push_back(INFINITY);
-                ++b;
-            }
-        }
-    }
-    // second layer of the pair store, ascending by t
-    const i64 nr = (i64)out.piv_t.size();
-    std::vector<i64> order((size_t)nr);
-    for (i64 i = 0; i < nr; ++i) order[i] = i;
-    std::sort(order.begin(), order.end(), [&](i64 x, i64 y) { return out.piv_t[x] < out.piv_t[y]; });
-    std::vector<u64> t((size_t)nr), sv((size_t)nr);
-    for (i64 i = 0; i < nr; ++i) { t[i] = out.piv_t[order[i]]; sv[i] = out.piv_s[order[i]]; }
-    double t3 = now_ms();
-    RC(ensure(c, s.red_t, (size_t)nr * 8));
-    RC(ensure(c, s.red_s, (size_t)nr * 8));
-    if (nr) {
-        CU(cudaMemcpy(s.red_t.p, t.data(), (size_t)nr * 8, cudaMemcpyHostToDevice));
-        CU(cudaMemcpy(s.red_s.p, sv.data(), (size_t)nr * 8, cudaMemcpyHostToDevice));
-    }
-    s.tim.reduce_xfer_ms += (float)(now_ms() - t3);
-    s.n_red = nr;
-    s.stats.n_reduced_pivots = nr;
-    s.stats.n_essential = (i64)out.ess_s.size();
-    s.stats.n_additions = out.additions;
+    s.n_red = n_piv;
+    s.stats.n_reduced_pivots = n_piv;
+    s.stats.n_essential = n_ess;
+    s.stats.n_additions = n_adds;
     s.stats.n_bars = (i64)s.bars.size() / 2;
     s.have_red = true;
     return RIPS_OK;
@@ -693,7 +819,8 @@ int check_dim(rips_ctx* c, int d, int lo)
 void free_dim(rips_ctx* c, DimState& s)
 {
     DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.pairsA, &s.pairsB, &s.irrA, &s.irrB, &s.nonA, &s.nonB,
-                     &s.pair_scratch, &s.pre_piv, &s.pre_adds, &s.red_t,
+                     &s.pair_scratch, &s.rd_piv, &s.rd_colref, &s.rd_todo, &s.rd_htk, &s.rd_htv, &s.rd_arena, &s.rd_cnt,
+                     &s.rd_rec, &s.rd_rec2, &s.rd_bars, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
     if (s.ev_made) for (int i = 0; i < EV_COUNT; ++i) cudaEventDestroy(s.ev[i]);
@@ -703,43 +830,43 @@ void free_dim(rips_ctx* c, DimState& s)
 int init_device_tables(rips_ctx* c, const float* dist_lower)
 {
     const i64 E = c->E, n = c->n;
-    CU(cudaMalloc(&c->d_counters, 64));
-    CU(cudaMalloc(&c->d_tickets, 32));
-    CU(cudaMallocHost(&c->h_counters, 64));
-    CU(cudaMalloc(&c->d_binom, c->h_binom.size() * 8));
-    c->dev_bytes += (i64)c->h_binom.size() * 8 + 96;
+    RC(ensure(c, c->b_counters, 256));
+    RC(ensure(c, c->b_tickets, 32));
+    c->d_counters = (u64*)c->b_counters.p;
+    c->d_tickets = (u32*)c->b_tickets.p;
+    CU(cudaMallocHost(&c->h_counters, 256));
+    RC(ensure(c, c->b_binom, c->h_binom.size() * 8));
+    c->d_binom = (u64*)c->b_binom.p;
     CU(cudaMemcpyAsync(c->d_binom, c->h_binom.data(), c->h_binom.size() * 8, cudaMemcpyHostToDevice, c->stream));
     const size_t eb = (size_t)(E ? E : 1);
-    CU(cudaMalloc(&c->d_dist, eb * 4));
-    CU(cudaMalloc(&c->d_edges, eb * 8));
-    CU(cudaMalloc(&c->d_K, eb * 4));
-    CU(cudaMalloc(&c->d_values, eb * 4));
-    c->dev_bytes += (i64)eb * 20;
+    RC(ensure(c, c->b_dist, eb * 4));
+    RC(ensure(c, c->b_edges, eb * 8));
+    RC(ensure(c, c->b_K, eb * 4));
+    RC(ensure(c, c->b_values, eb * 4));
+    c->d_dist = (float*)c->b_dist.p;
+    c->d_edges = (u64*)c->b_edges.p;
+    c->d_K = (u32*)c->b_K.p;
+    c->d_values = (float*)c->b_values.p;
     c->n_distinct = 0;
     if (E > 0) {
         CU(cudaMemcpyAsync(c->d_dist, dist_lower, (size_t)E * 4, cudaMemcpyDefault, c->stream));
-        u64* tmp = nullptr;
-        CU(cudaMalloc(&tmp, (size_t)E * 8));
+        RC(ensure(c, c->b_init_tmp, (size_t)E * 8));
         CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
         CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
         CU(launch_prep_edges(c->d_dist, E, c->d_edges, (int*)(c->d_counters + 1), c->stream));
         SortPlan plan = sort_make_plan(32, 64);
         RC(ensure(c, c->sort_scratch, sort_scratch_bytes(E, plan)));
         u64* res = nullptr;
-        cudaError_t e = sort_u64(c->d_edges, tmp, E, plan, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches);
-        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(e, "edge sort"); }
-        if (res != c->d_edges) { u64* t = c->d_edges; c->d_edges = res; tmp = t; }
-        DevBuf status;
-        int r = ensure(c, status, (size_t)rank_edges_tiles(E) * 8);
-        if (r != RIPS_OK) { cudaFree(tmp); return r; }
-        cudaMemsetAsync(status.p, 0, (size_t)rank_edges_tiles(E) * 8, c->stream);
-        e = launch_rank_edges(c->d_edges, E, c->d_K, c->d_values, (u64*)status.p, c->d_tickets, c->d_counters, c->stream);
+        CU(sort_u64(c->d_edges, (u64*)c->b_init_tmp.p, E, plan, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        if (res != c->d_edges) { std::swap(c->b_edges, c->b_init_tmp); c->d_edges = (u64*)c->b_edges.p; }
+        RC(ensure(c, c->b_init_status, (size_t)rank_edges_tiles(E) * 8));
+        CU(cudaMemsetAsync(c->b_init_status.p, 0, (size_t)rank_edges_tiles(E) * 8, c->stream));
+        CU(launch_rank_edges(c->d_edges, E, c->d_K, c->d_values, (u64*)c->b_init_status.p, c->d_tickets, c->d_counters, c->stream));
         c->launches += 2;
-        if (e == cudaSuccess) e = cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-        cudaFree(tmp);
-        release(c, status);
-        if (e != cudaSuccess) return cuda_fail(e, "edge ranking");
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        release(c, c->b_init_tmp);
+        release(c, c->b_init_status);
         if ((int)c->h_counters[1] != 0) {
             g_last_error = "rips_init: the distance matrix holds a NaN, negative or infinite entry";
             return RIPS_EINVAL;
@@ -757,9 +884,8 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         else if ((pitch & 1) == 0) ++pitch;
         c->kf_pitch = pitch;
         const size_t kf_bytes = (((size_t)n * (size_t)pitch * (c->kf_u16 ? 2 : 4)) + 15) & ~(size_t)15;
-        cudaError_t e = cudaMalloc(&c->d_Kf, kf_bytes);
-        if (e != cudaSuccess) { cudaGetLastError(); g_last_error = "cudaMalloc of the full key matrix failed"; return RIPS_ENOMEM; }
-        c->dev_bytes += (i64)kf_bytes;
+        RC(ensure(c, c->b_Kf, kf_bytes));
+        c->d_Kf = c->b_Kf.p;
         CU(cudaMemsetAsync(c->d_Kf, 0, kf_bytes, c->stream));
         CU(launch_build_full_keys(c->d_K, (int)n, pitch, c->d_Kf, c->kf_u16, c->stream));
         c->launches += 1;
@@ -775,6 +901,30 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
     c->thr_key = lo;
     c->key_bits = bits_for(c->n_distinct); // the value n_distinct itself is the key of the column sentinel
     return RIPS_OK;
+}
+
+// Device bytes rips_init holds for n points (distances, edge records and their sort buffer, keys, values, the full
+// key matrix as u32, binomial table, counters, the edge sort's scratch): an upper bound.
+size_t setup_bytes(i64 n, int kmax)
+{
+    const size_t E = (size_t)(n * (n - 1) / 2) + 1;
+    SortPlan plan = sort_make_plan(32, 64);
+    return E * (4 + 8 + 8 + 4 + 4) + (size_t)n * (size_t)(n + 4) * 4 + (size_t)(kmax + 1) * (size_t)(n + 1) * 8 + sort_scratch_bytes((i64)E, plan) +
+           (E / 2048 + 1) * 8 + (size_t)n * 20 + (1 << 16);
+}
+
+// Device bytes one dimension with `cand` candidates can hold when a share `keep` of them survives the threshold:
+// column records and pair slots with their ping-pong buffers (4 x 8), the irregular-pair and non-apparent lists with
+// theirs (4 lists of max(4096, slots / 8) records), the clearing bitmap over ALL candidates, the look-back words of
+// three sorts (2048 bytes per tile of 5120 records) and their heads, the views the accessors materialise (filtration
+// 12, apparent pairs 16, pivots 16, non-apparent columns 12 / 8 bytes per column), the reduction's per-column words
+// (at most slots / 8 non-apparent columns) and its default arena.
+long double dim_bytes(long double cand, long double keep)
+{
+    const long double slots = std::max<long double>(4096.0L, cand * keep);
+    const long double lists = std::max<long double>(4096.0L, slots / 8);
+    return slots * 32 + lists * 8 * 4 + cand / 8 + 64 + 3 * ((slots / 5120 + 2) * 2048 + (1 << 15)) + slots * (12 + 16 + 16) + lists * 12 +
+           lists * 96 + std::max<long double>((long double)(256u << 20), slots * 64);
 }
 
 } // namespace
@@ -798,31 +948,27 @@ const char* rips_last_error(void) { return g_last_error.c_str(); }
 
 int rips_workspace_bytes(int64_t n, int dim_max, int64_t* bytes)
 {
+    g_last_error.clear();
     if (!bytes || n < 1 || dim_max < 0 || dim_max > 4) return RIPS_EINVAL;
     if (n > 46340) return RIPS_EOVERFLOW;
     std::vector<u64> b;
     build_binom(n, dim_max + 3, b);
-    auto C = [&](int k) { return b[(size_t)k * (n + 1) + n]; };
-    if (C(dim_max + 2) >> 62) return RIPS_EOVERFLOW;
-    long double total = 0;
-    const long double E = (long double)n * (n - 1) / 2;
-    // set-up: distances, edge records (+ sort buffer), lower-triangle keys, values, full key matrix, binomials
-    total += E * 36 + (long double)n * (n + 3) * 4 + (long double)b.size() * 8;
-    for (int d = 1; d <= dim_max; ++d) {
-        long double cand = (long double)C(d + 1);
-        // slot mode: column records and pair slots, each with its ping-pong buffer (4 x 8 bytes per candidate),
-        // the two small lists with theirs (2 x 2 x cand/8 records), the clearing bitmap, look-back words of the
-        // sorts (256 words per tile of 4608 records, two sorts in flight), sort scratch heads
-        total += cand * 32 + cand * 4 + cand / 8 + cand / 4608 * 256 * 8 * 2 + (3 << 16);
-    }
+    if (b[(size_t)(dim_max + 2) * (n + 1) + n] >> 62) return RIPS_EOVERFLOW;
+    long double total = (long double)setup_bytes(n, dim_max + 3);
+    for (int d = 1; d <= dim_max; ++d) total += dim_bytes((long double)b[(size_t)(d + 1) * (n + 1) + n], 1.0L);
+    total += total / 64 + (16 << 20); // granules of 256 bytes, holes left by lists that had to grow
     if (total > 9.0e18L) return RIPS_EOVERFLOW;
     *bytes = (int64_t)total;
     return RIPS_OK;
 }
 
-int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* stream)
+int64_t rips_last_required_bytes(void) { return g_required_bytes; }
+
+int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* workspace_dev,
+              int64_t workspace_bytes, void* stream)
 {
     g_last_error.clear();
+    g_required_bytes = 0;
     if (!out) return RIPS_EINVAL;
     *out = nullptr;
     if (n < 1 || dim_max < 0 || dim_max > 4 || std::isnan(threshold)) return RIPS_EINVAL;
@@ -843,18 +989,54 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     c->threshold = threshold;
     c->stream = (cudaStream_t)stream;
     c->kmax = dim_max + 3;
-    if (!getenv("RIPS_ONE_STREAM")) {
-        if (cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream2 = nullptr; }
-        if (cudaStreamCreateWithFlags(&c->stream3, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream3 = nullptr; }
-        if (cudaEventCreateWithFlags(&c->ev_join3, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join3 = nullptr; c->stream3 = nullptr; }
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
+        if (c->sms < 1) c->sms = 1;
     }
+    if (cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream2 = nullptr; }
+    if (cudaStreamCreateWithFlags(&c->stream3, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); c->stream3 = nullptr; }
+    if (cudaEventCreateWithFlags(&c->ev_join3, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join3 = nullptr; c->stream3 = nullptr; }
     if (cudaEventCreateWithFlags(&c->ev_fused, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_fused = nullptr; c->stream2 = nullptr; }
     if (cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->ev_join = nullptr; c->stream2 = nullptr; }
-    if (const char* e = getenv("RIPS_FAST_VISITS")) c->fast_visits = atoi(e);
     build_binom(n, c->kmax, c->h_binom);
     if (hbinom(c, n, dim_max + 2) >> 62) { delete c; return RIPS_EOVERFLOW; }
     c->dims.resize((size_t)dim_max + 2);
-    int r = init_device_tables(c, dist_lower);
+    int r = RIPS_OK;
+    if (workspace_dev) {
+        if (workspace_bytes < 4096 || ((uintptr_t)workspace_dev & 255)) {
+            g_last_error = "rips_init: the workspace must be 256-byte aligned and at least 4096 bytes";
+            delete c;
+            return RIPS_EINVAL;
+        }
+        c->pool.add_chunk(workspace_dev, (size_t)workspace_bytes, false);
+    } else {
+        // the library's own workspace: first what the set-up needs (known from n), the rest once the threshold's
+        // share of admissible edges is known
+        void* base = nullptr;
+        const size_t sb = Pool::round(setup_bytes(n, c->kmax));
+        cudaError_t e2 = cudaMalloc(&base, sb);
+        if (e2 != cudaSuccess) { cudaGetLastError(); g_last_error = "rips_init: cudaMalloc of the set-up workspace failed"; delete c; return RIPS_ENOMEM; }
+        c->pool.add_chunk(base, sb, true);
+        c->pool.may_grow = true;
+    }
+    r = init_device_tables(c, dist_lower);
+    if (r == RIPS_OK && !workspace_dev) {
+        const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
+        long double rest = 0;
+        for (int d = 1; d <= dim_max; ++d) {
+            const double surv = std::pow(q, (double)((d + 1) * d / 2));
+            const bool compact = c->thr_key != 0 && surv < 0.5; // the rule of run_stage1
+            rest += dim_bytes((long double)hbinom(c, n, d + 1), compact ? std::min(1.0, 2.0 * surv) : 1.0);
+        }
+        rest += rest / 64 + (16 << 20);
+        size_t free_b = 0, total_b = 0;
+        cudaMemGetInfo(&free_b, &total_b);
+        if (rest > (long double)free_b * 0.9L) rest = (long double)free_b * 0.9L;
+        void* base = nullptr;
+        if (cudaMalloc(&base, (size_t)rest) == cudaSuccess) c->pool.add_chunk(base, (size_t)rest, true);
+        else cudaGetLastError(); // chunks are added as the computation asks for them
+    }
     if (r == RIPS_OK) {
         // the widest record of the requested dimensions must fit 64 bits
         int lb = (dim_max + 1) * c->vbits;
@@ -882,14 +1064,10 @@ void rips_free(rips_ctx* c)
     release(c, c->d0_pairs);
     release(c, c->d0_death);
     release(c, c->d0_uf);
-    cudaFree(c->d_dist);
-    cudaFree(c->d_edges);
-    cudaFree(c->d_K);
-    cudaFree(c->d_Kf);
-    cudaFree(c->d_values);
-    cudaFree(c->d_binom);
-    cudaFree(c->d_counters);
-    cudaFree(c->d_tickets);
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    else cudaDeviceSynchronize();
+    for (Pool::Chunk& ch : c->pool.chunks)
+        if (ch.owned) cudaFree(ch.base);
     if (c->h_counters) cudaFreeHost(c->h_counters);
     cudaGetLastError();
     delete c;
@@ -1084,7 +1262,15 @@ int rips_timings(rips_ctx* c, int d, rips_timings_t* out)
 int rips_device_bytes(rips_ctx* c, int64_t* bytes)
 {
     if (!c || !bytes) return RIPS_EINVAL;
-    *bytes = c->dev_bytes;
+    *bytes = (int64_t)c->pool.total();
+    return RIPS_OK;
+}
+
+int rips_workspace_in_use(rips_ctx* c, int64_t* bytes, int64_t* peak)
+{
+    if (!c || !bytes) return RIPS_EINVAL;
+    *bytes = (int64_t)c->pool.in_use;
+    if (peak) *peak = (int64_t)c->pool.peak;
     return RIPS_OK;
 }
 

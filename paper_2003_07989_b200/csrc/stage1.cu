@@ -21,8 +21,6 @@
 //     coalesced stores.  With a threshold survivors are compacted in increasing index with a
 //     warp-level decoupled look-back.
 //   * the digit histograms of the two sorts that follow are accumulated on the way out.
-#include <cstdlib>
-
 #include "apparent.cuh"
 #include "kernels.cuh"
 
@@ -438,8 +436,7 @@ template <int M, typename KT>
 cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 {
     const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
-    static const bool kf_global = getenv("RIPS_KF_GLOBAL") != nullptr; // tuning: never stage Kf in shared memory
-    const int k_in = (!kf_global && !p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
+    const int k_in = (!p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
     const size_t smem = (k_in ? kf_bytes : 0) +
                         ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.stage_cap * 8 : 0);
     auto kern = k_in ? enumerate_apparent_kernel<M, KT, true> : enumerate_apparent_kernel<M, KT, false>;

@@ -21,15 +21,16 @@ RIPS_OK, RIPS_EINVAL, RIPS_EOVERFLOW, RIPS_ENOMEM, RIPS_ECUDA = 0, -1, -2, -3, -
 SYMBOLS = [
     "rips_workspace_bytes", "rips_init", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce", "rips_import_pivots",
     "rips_barcodes", "rips_filtration", "rips_apparent_pairs", "rips_nonapparent", "rips_pivots",
-    "rips_pivot_lookup", "rips_stats", "rips_timings", "rips_device_bytes", "rips_kernel_launches",
-    "rips_sort_u64", "rips_strerror", "rips_last_error", "rips_free",
+    "rips_pivot_lookup", "rips_stats", "rips_timings", "rips_device_bytes", "rips_workspace_in_use", "rips_kernel_launches",
+    "rips_sort_u64", "rips_strerror", "rips_last_error", "rips_last_required_bytes", "rips_free",
 ]
 
 
 class RipsStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in (
         "n_candidates", "n_removed_by_diameter", "n_cleared", "n_columns", "n_apparent", "n_nonapparent",
-        "n_reduced_pivots", "n_essential", "n_additions", "n_bars", "n_slots", "n_regular")] + [(k, C.c_int32) for k in (
+        "n_reduced_pivots", "n_essential", "n_additions", "n_bars", "n_slots", "n_regular", "n_reduce_serial",
+        "n_reduce_displaced", "reduce_arena_bytes")] + [(k, C.c_int32) for k in (
         "key_bits", "index_bits", "sort_passes", "pair_sort_passes")]
 
     def as_dict(self):
@@ -66,7 +67,7 @@ def lib():
         pp = C.POINTER(C.c_void_p)
         pi64 = C.POINTER(C.c_int64)
         l.rips_workspace_bytes.argtypes = [i64, i32, pi64]
-        l.rips_init.argtypes = [pp, vp, i64, i32, C.c_float, vp]
+        l.rips_init.argtypes = [pp, vp, i64, i32, C.c_float, vp, i64, vp]
         for f in ("rips_compute", "rips_dim0"):
             getattr(l, f).argtypes = [vp]
         for f in ("rips_stage1", "rips_stage2", "rips_reduce"):
@@ -81,6 +82,9 @@ def lib():
         l.rips_timings.argtypes = [vp, i32, C.POINTER(RipsTimings)]
         l.rips_device_bytes.argtypes = [vp, pi64]
         l.rips_kernel_launches.argtypes = [vp, pi64]
+        l.rips_workspace_in_use.argtypes = [vp, pi64, pi64]
+        l.rips_last_required_bytes.argtypes = []
+        l.rips_last_required_bytes.restype = C.c_int64
         l.rips_sort_u64.argtypes = [vp, vp, i64, i32, i32, vp]
         l.rips_strerror.argtypes = [i32]
         l.rips_strerror.restype = C.c_char_p
@@ -125,6 +129,10 @@ def rips_workspace_bytes(n, dim_max):
     return b.value
 
 
+def rips_last_required_bytes():
+    return int(lib().rips_last_required_bytes())
+
+
 def rips_sort_u64(keys, lo_bit, hi_bit):
     """In-place stable sort of a torch int64 CUDA tensor (read as uint64) on bits [lo_bit, hi_bit)."""
     torch = _torch()
@@ -138,7 +146,9 @@ def rips_sort_u64(keys, lo_bit, hi_bit):
 class Rips:
     """One context = one distance matrix.  Methods mirror the C entry points (rips_<method>)."""
 
-    def __init__(self, dist_lower, n, dim_max, threshold=float("inf"), stream=None):
+    def __init__(self, dist_lower, n, dim_max, threshold=float("inf"), stream=None, workspace=None):
+        """workspace: None = the library allocates its own; an int = that many bytes of torch device memory; a torch
+        uint8 CUDA tensor = that memory (it must outlive the context, which keeps a reference)."""
         torch = _torch()
         l = lib()
         self._h = C.c_void_p()
@@ -152,7 +162,12 @@ class Rips:
         assert self._keep.size == n * (n - 1) // 2 if not hasattr(self._keep, "numel") else self._keep.numel() == n * (n - 1) // 2
         if stream is None and torch.cuda.is_available():
             stream = torch.cuda.current_stream().cuda_stream
-        _check(l.rips_init(C.byref(self._h), ptr if n > 1 else None, n, dim_max, threshold, stream or None), "rips_init")
+        if isinstance(workspace, int):
+            workspace = torch.empty(workspace, dtype=torch.uint8, device="cuda")
+        self._workspace = workspace
+        wptr, wbytes = (workspace.data_ptr(), workspace.numel()) if workspace is not None else (None, 0)
+        _check(l.rips_init(C.byref(self._h), ptr if n > 1 else None, n, dim_max, threshold, wptr, wbytes, stream or None),
+               "rips_init")
 
     # -- life cycle
     def free(self):
@@ -245,6 +260,12 @@ class Rips:
         b = C.c_int64()
         _check(lib().rips_device_bytes(self._h, C.byref(b)), "rips_device_bytes")
         return b.value
+
+    def workspace_in_use(self):
+        """(bytes handed out now, peak)"""
+        a, b = C.c_int64(), C.c_int64()
+        _check(lib().rips_workspace_in_use(self._h, C.byref(a), C.byref(b)), "rips_workspace_in_use")
+        return a.value, b.value
 
     def kernel_launches(self):
         b = C.c_int64()

@@ -34,8 +34,8 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_sizes_match_header():
     from paper_2003_07989_b200 import rips
-    # rips_stats_t: 12 int64 + 4 int32; rips_timings_t: 13 floats
-    assert ctypes.sizeof(rips.RipsStats) == 12 * 8 + 4 * 4
+    # rips_stats_t: 15 int64 + 4 int32; rips_timings_t: 13 floats
+    assert ctypes.sizeof(rips.RipsStats) == 15 * 8 + 4 * 4
     assert ctypes.sizeof(rips.RipsTimings) == 13 * 4
     text = open(os.path.join(ROOT, "include", "rips.h")).read()
     stats = re.search(r"typedef struct \{(.*?)\} rips_stats_t;", text, flags=re.S).group(1)
@@ -55,8 +55,9 @@ def test_host_only_error_paths(lib):
     assert lib.rips_workspace_bytes(60000, 4, ctypes.byref(b)) == rips.RIPS_EOVERFLOW
     assert lib.rips_strerror(rips.RIPS_ECUDA).decode() == "CUDA error"
     h = ctypes.c_void_p()
-    assert lib.rips_init(ctypes.byref(h), None, 0, 1, 1.0, None) == rips.RIPS_EINVAL
-    assert lib.rips_init(ctypes.byref(h), None, 5, 9, 1.0, None) == rips.RIPS_EINVAL
+    assert lib.rips_init(ctypes.byref(h), None, 0, 1, 1.0, None, 0, None) == rips.RIPS_EINVAL
+    assert lib.rips_init(ctypes.byref(h), None, 5, 9, 1.0, None, 0, None) == rips.RIPS_EINVAL
+    assert lib.rips_last_required_bytes() == 0
     assert lib.rips_compute(None) == rips.RIPS_EINVAL
 
 

@@ -189,14 +189,73 @@ def test_more_than_256_vertices(R):
     check_against_oracle(R, w.dist, w.n, 2, thr, "n = 300, dimension 2, 5 % of the edges")
 
 
-def test_workspace_estimate_bounds_what_is_held(R):
-    """rips_workspace_bytes is an upper bound of rips_device_bytes after rips_compute (accessor views excluded)."""
-    for k, n in [(1, 50), (2, 60), (5, 120)]:
+def _everything(g, D):
+    out = [g.barcodes(0)]
+    for d in range(1, D + 1):
+        out += [g.filtration(d), g.apparent_pairs(d), g.nonapparent(d), g.pivots(d), g.barcodes(d)]
+    return out
+
+
+def test_caller_workspace(R):
+    """rips_init with a caller's workspace of rips_workspace_bytes: rips_compute and every accessor fit, the
+    context's device bytes are that workspace and never change, the results are the library-owned ones."""
+    import torch
+    for k, n in [(1, 50), (2, 60), (5, 120), (4, 200)]:
         w = inputs.config(k, n)
         thr = w.threshold if k != 5 else inputs.enclosing_radius(w.dist, n)
-        with R.Rips(w.dist, n, w.dim_max, thr) as g:
+        size = R.rips_workspace_bytes(n, w.dim_max)
+        ws = torch.empty(size, dtype=torch.uint8, device="cuda")
+        with R.Rips(w.dist, n, w.dim_max, thr, workspace=ws) as g, R.Rips(w.dist, n, w.dim_max, thr) as h:
+            assert g.device_bytes() == size // 256 * 256
+            g.compute(); h.compute()
+            a, b = _everything(g, w.dim_max), _everything(h, w.dim_max)
+            assert g.device_bytes() == size // 256 * 256
+            used, peak = g.workspace_in_use()
+            assert 0 < used <= peak <= size
+            for x, y in zip(a, b):
+                if isinstance(x, tuple):
+                    assert all(bool((p == q).all()) for p, q in zip(x, y))
+                else:
+                    assert np.array_equal(x, y)
+            # the hot path again on the same context: no growth
+            for d in range(1, w.dim_max + 1):
+                g.stage1(d); g.stage2(d)
+            assert g.workspace_in_use()[1] <= size
+
+
+def test_workspace_too_small(R):
+    """A workspace that cannot hold the computation: RIPS_ENOMEM with the size that would have fitted, nothing
+    crashes, and a workspace of the reported size gets further."""
+    import torch
+    w = inputs.config(2, 60)
+    with pytest.raises(R.RipsError) as e:
+        R.Rips(w.dist, w.n, w.dim_max, w.threshold, workspace=8192)          # not even the set-up
+    assert e.value.code == R.RIPS_ENOMEM and R.rips_last_required_bytes() > 8192
+    with pytest.raises(R.RipsError) as e:
+        R.Rips(w.dist, w.n, w.dim_max, w.threshold, workspace=torch.empty(5000, dtype=torch.uint8, device="cuda")[1:])
+    assert e.value.code == R.RIPS_EINVAL                                    # misaligned
+    size = 2 << 20                                                          # the set-up fits, dimension 3 does not
+    for _ in range(40):
+        g = R.Rips(w.dist, w.n, w.dim_max, w.threshold, workspace=size)
+        try:
             g.compute()
-            assert 0 < g.device_bytes() <= R.rips_workspace_bytes(n, w.dim_max), (k, n)
+            _everything(g, w.dim_max)
+            break
+        except R.RipsError as err:
+            assert err.code == R.RIPS_ENOMEM
+            need = R.rips_last_required_bytes()
+            assert need > size
+            size = max(need, size + size // 2)   # the report covers the request that failed, not the ones after it
+        finally:
+            g.free()
+    else:
+        raise AssertionError("the reported sizes never sufficed")
+    assert size <= 2 * R.rips_workspace_bytes(w.n, w.dim_max)     # (the loop grows geometrically)
+    o = oracle.barcodes(w.dist, w.n, w.dim_max, w.threshold)
+    with R.Rips(w.dist, w.n, w.dim_max, w.threshold, workspace=size) as g:
+        g.compute()
+        for d in range(1, w.dim_max + 1):
+            assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32))
 
 
 def test_two_contexts_interleaved_and_repeated_stages(R):
