@@ -318,9 +318,12 @@ SortPlan sort_make_plan(int lo_bit, int hi_bit)
     int np = (total + 7) / 8; // digits of at most 8 bits (RIPS_SORT_MAX_BINS = 256)
     if (np > RIPS_SORT_MAX_PASSES) np = RIPS_SORT_MAX_PASSES; // callers never ask for more than 64 bits
     p.npasses = np;
-    int basew = total / np, extra = total % np, at = lo_bit;
+    // 8-bit digits from the bottom, the last one takes what is left: a producer kernel that accumulates the
+    // histograms (FusedHist) then takes digit r of a field as byte r of it, with no shift or mask tables
+    int at = lo_bit;
     for (int i = 0; i < np; ++i) {
-        int w = basew + (i < extra ? 1 : 0);
+        int w = (hi_bit - at) < 8 ? (hi_bit - at) : 8;
+        if (w < 1) w = 1;
         p.shift[i] = at;
         p.bits[i] = w;
         at += w;

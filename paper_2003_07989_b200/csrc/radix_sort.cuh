@@ -14,7 +14,7 @@ struct SortPlan {
     i64 tile_items;
 };
 
-// Digits covering bits [lo_bit, hi_bit): as few passes as 8-bit digits allow, widths balanced.
+// Digits covering bits [lo_bit, hi_bit): 8-bit digits from lo_bit up, the last one narrower (digit r = byte r of the field).
 SortPlan sort_make_plan(int lo_bit, int hi_bit);
 
 // Scratch the sort needs besides the ping-pong buffer, in bytes (status words, histograms, ticket).

@@ -585,7 +585,8 @@ int run_stage1(rips_ctx* c, int d)
         irr_cap = std::max(irr_cap, ni); // rare: more irregular pairs / non-apparent columns than provisioned; run again
         non_cap = std::max(non_cap, nn);
     }
-    s.len = (i64)c->h_counters[S1C_KEPT];
+    // (slot mode counts what it drops; the columns are the rest)
+    s.len = s.compact ? (i64)c->h_counters[S1C_KEPT] : (i64)(s.total - c->h_counters[S1C_OVER] - c->h_counters[S1C_CLEARED]);
     s.slots = s.compact ? s.len : (i64)s.total;
     s.n_reg = (i64)c->h_counters[S1C_REGULAR];
     s.n_irr = (i64)c->h_counters[S1C_IRREGULAR];

@@ -423,6 +423,293 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same steps for SLOT mode only (every candidate keeps its slot: no threshold, or one that keeps most), written
+// for the instruction budget: the kernel is bound by instruction issue, so what is warp- or slab-uniform is taken out
+// of the per-candidate path.
+//   * per slab, U2[w] = min_{j>=2} key1(v_j, w) for every vertex w, in a per-warp row of shared memory: key(s) is then
+//     min(up2, U2[v1], U2[x], Kf[v1][x]) -- three gathers instead of 2(M-2)+1 -- and the same row is the shared part of
+//     every cofacet test of the slab;
+//   * row offsets v1*pitch and x*pitch are carried along by lane_advance (additions only);
+//   * the cofacet scan tests the first four vertices n-1..n-4 of every lane at once, branch-free (the mean number of
+//     visits is about two: one lane-serial loop made the whole warp wait for its slowest lane), then four more for the
+//     warps that still have an open lane, then the warp-cooperative scan of the general kernel;
+//   * digits of the fused histograms are taken from the 32-bit key / cofacet vertex, not from the 64-bit records;
+//   * C(v, M+1), the offset of a regular pair's row, comes from a copy of that binomial column in shared memory;
+//   * nothing is counted per warp step: the number of columns is total - over - cleared.
+// Same records, same lists, same counters as enumerate_apparent_kernel (the tests compare both with the oracle).
+// ---------------------------------------------------------------------------------------------------------------
+template <int M, typename KT, bool KS>
+__global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1Params p)
+{
+    extern __shared__ __align__(16) unsigned char smem1[];
+    __shared__ u32 s_hist_cols[S1_MAX_FUSED][256];
+    __shared__ u32 s_hist_pairs[S1_MAX_FUSED_P][256];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n = p.n, pitch = p.pitch;
+
+    // ---- shared memory: [Kf (KS)] [C(., M+1) : n u64] [U2 : S1_WARPS rows of n KT (M > 2)]
+    size_t off_b = 0;
+    const KT* __restrict__ Kf;
+    if (KS) {
+        const int cnt16 = (int)(((size_t)n * pitch * sizeof(KT) + 15) / 16);
+        uint4* dst = reinterpret_cast<uint4*>(smem1);
+        const uint4* src = reinterpret_cast<const uint4*>(p.Kf);
+        for (int i = tid; i < cnt16; i += S1_THREADS) dst[i] = __ldg(src + i);
+        Kf = reinterpret_cast<const KT*>(smem1);
+        off_b = (size_t)cnt16 * 16;
+    } else {
+        Kf = reinterpret_cast<const KT*>(p.Kf);
+    }
+    u64* const sprec = reinterpret_cast<u64*>(smem1 + off_b); // record of a regular pair with cofacet vertex v, minus cidx(s)
+    for (int i = tid; i < n; i += S1_THREADS) sprec[i] = ((u64)(u32)i << p.tbits) + p.bt(i, M + 1);
+    off_b += (size_t)n * 8;
+    KT* const u2 = reinterpret_cast<KT*>(smem1 + off_b) + (size_t)warp * ((n + 7) & ~7);
+    for (int i = tid; i < S1_MAX_FUSED * 256; i += S1_THREADS) (&s_hist_cols[0][0])[i] = 0;
+    for (int i = tid; i < S1_MAX_FUSED_P * 256; i += S1_THREADS) (&s_hist_pairs[0][0])[i] = 0;
+    __syncthreads();
+
+    // digits of the two sorts: byte r of the 32-bit key / cofacet vertex (sort_make_plan: 8-bit digits from the
+    // bottom of the field)
+    const int ncd = p.fh_cols.hist ? p.fh_cols.npasses : 0, npd = p.fh_pairs.hist ? p.fh_pairs.npasses : 0;
+    const u32 thr1 = p.thr_key + 1u;
+    const u32 sentinel_key = p.sentinel_key;
+    const int vbits = p.vbits, lowbits = p.lowbits;
+    const u32 vmul = 1u << vbits;
+    const u64 psentinel = (u64)(u32)n << p.tbits;
+    u32 n_clr = 0, n_reg = 0;
+    u64 n_over = 0;
+
+    for (;;) {
+        u32 chunk = 0;
+        if (lane == 0) chunk = atomicAdd(p.ticket, 1u);
+        chunk = __shfl_sync(RIPS_FULL_MASK, chunk, 0);
+        if ((i64)chunk >= p.tiles) break;
+        u64 idx = (u64)chunk * (u64)p.chunk;
+        int rem = (p.total - idx) < (u64)p.chunk ? (int)(p.total - idx) : p.chunk;
+        int v[M];
+        decode_simplex_fast<M>(p.bt, idx, n, v); // warp-uniform
+        i64 e0 = (i64)v[1] * (v[1] - 1) / 2 + v[0];
+
+        while (rem > 0) {
+            // ---- per slab (warp-uniform)
+            u32 up2 = 0xffffffffu;
+#pragma unroll
+            for (int a = 3; a < M; ++a)
+#pragma unroll
+                for (int b = 2; b < a; ++b) up2 = min(up2, (u32)Kf[v[a] * pitch + v[b]]);
+            u64 slab_low = 0;
+#pragma unroll
+            for (int j = M - 1; j >= 2; --j) slab_low = (slab_low << vbits) | (u64)(u32)v[j];
+            slab_low <<= 2 * vbits;
+            const i64 slab_len = (M > 2) ? (i64)v[M > 2 ? 2 : 1] * (v[M > 2 ? 2 : 1] - 1) / 2 : (i64)n * (n - 1) / 2;
+            const int seg = (slab_len - e0) < (i64)rem ? (int)(slab_len - e0) : rem;
+            u32 ur0 = 0xffffffffu, ur1 = 0xffffffffu, ur2 = 0xffffffffu, ur3 = 0xffffffffu;
+            if (M > 2) {
+                __syncwarp();
+                for (int w = lane; w < n; w += 32) {
+                    u32 u = 0xffffffffu;
+#pragma unroll
+                    for (int j = 2; j < M; ++j) u = min(u, (u32)Kf[v[j] * pitch + w]);
+                    u2[w] = (KT)u; // a diagonal zero stays zero: vertices of the slab fail every test by themselves
+                }
+                __syncwarp();
+                ur0 = n >= 1 ? (u32)u2[n - 1] : 0u;
+                ur1 = n >= 2 ? (u32)u2[n - 2] : 0u;
+                ur2 = n >= 3 ? (u32)u2[n - 3] : 0u;
+                ur3 = n >= 4 ? (u32)u2[n - 4] : 0u;
+            } else {
+                if (n < 4) ur3 = 0u;
+                if (n < 3) ur2 = 0u;
+                if (n < 2) ur1 = 0u;
+            }
+            const int vtop_slab = (M > 2) ? v[M - 1] : 0;
+
+            // ---- the lanes walk the segment's pairs (v1, x) in index order, 32 at a time
+            int lv1, lx;
+            {
+                const i64 e = e0 + lane;
+                lv1 = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)e)) * 0.5f);
+                if (lv1 < 1) lv1 = 1;
+                while ((i64)lv1 * (lv1 - 1) / 2 > e) --lv1;
+                while ((i64)(lv1 + 1) * lv1 / 2 <= e) ++lv1;
+                lx = (int)(e - (i64)lv1 * (lv1 - 1) / 2);
+            }
+            int r1o = lv1 * pitch, xo = lx * pitch; // row offsets, carried along
+            const int pitch32 = 32 * pitch;
+            for (int off = lane; off - lane < seg; off += 32) {
+                const bool valid = off < seg;
+                const u64 ci = idx + (u64)off;
+                // ---- a3/a4: key of the simplex, threshold, clearing
+                bool keep = false;
+                u32 key1 = up2;
+                if (valid) {
+                    if (M > 2) key1 = min(min(key1, (u32)u2[lv1]), (u32)u2[lx]);
+                    key1 = min(key1, (u32)Kf[r1o + lx]);
+                    if (key1 >= thr1) {
+                        bool clr;
+                        if (p.clear.bitmap) clr = (__ldg(p.clear.bitmap + (ci >> 5)) >> ((u32)ci & 31u)) & 1u;
+                        else
+                            clr = in_sorted(p.clear.layer1, p.clear.n1, p.clear.shift1, ci) ||
+                                  in_sorted(p.clear.layer2, p.clear.n2, 0, ci);
+                        keep = !clr;
+                        n_clr += clr;
+                    } else
+                        ++n_over;
+                }
+                // ---- a7: cofacet vertices n-1 .. n-4 for every lane at once
+                int fv = -1;
+                {
+                    const KT* a = Kf + r1o + (n - 1);
+                    const KT* b = Kf + xo + (n - 1);
+                    const bool h0 = min(min(ur0, (u32)a[0]), (u32)b[0]) >= key1;
+                    const bool h1 = n >= 2 && min(min(ur1, (u32)a[n >= 2 ? -1 : 0]), (u32)b[n >= 2 ? -1 : 0]) >= key1;
+                    const bool h2 = n >= 3 && min(min(ur2, (u32)a[n >= 3 ? -2 : 0]), (u32)b[n >= 3 ? -2 : 0]) >= key1;
+                    const bool h3 = n >= 4 && min(min(ur3, (u32)a[n >= 4 ? -3 : 0]), (u32)b[n >= 4 ? -3 : 0]) >= key1;
+                    fv = h0 ? n - 1 : h1 ? n - 2 : h2 ? n - 3 : h3 ? n - 4 : -1;
+                    if (!keep) fv = -1;
+                }
+                u32 open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
+                if (open && n > 4) { // four more for the lanes still open
+                    const int kend = n < 8 ? n : 8;
+                    if (keep && fv < 0) {
+                        for (int k = 4; k < kend; ++k) {
+                            const u32 uu = (M > 2) ? (u32)u2[n - 1 - k] : 0xffffffffu;
+                            if (min(min(uu, (u32)Kf[r1o + n - 1 - k]), (u32)Kf[xo + n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
+                        }
+                    }
+                    open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
+                    // the rest by the whole warp, one open lane after the other, 32 cofacet vertices per step
+                    while (open) {
+                        const int src = __ffs(open) - 1;
+                        open &= open - 1;
+                        const int xs = __shfl_sync(RIPS_FULL_MASK, xo, src);
+                        const int v1s = __shfl_sync(RIPS_FULL_MASK, r1o, src);
+                        const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
+                        int res = -1;
+                        for (int base = n - 1 - kend; base >= 0; base -= 32) {
+                            const int vv = base - lane;
+                            bool ok = false;
+                            if (vv >= 0) {
+                                u32 m = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                                if (M > 2) m = min(m, (u32)u2[vv]);
+                                ok = m >= ks;
+                            }
+                            const u32 bb = __ballot_sync(RIPS_FULL_MASK, ok);
+                            if (bb) { res = base - (__ffs(bb) - 1); break; }
+                        }
+                        if (lane == src) fv = res;
+                    }
+                }
+                const bool found = fv >= 0;
+                const int vtop = (M > 2) ? vtop_slab : lv1;
+                const bool regular = found && fv > vtop;
+                const u32 kk = keep ? key1 - 1u : sentinel_key;
+                const u32 fvv = regular ? (u32)fv : (u32)n;
+                u64 prec = psentinel;
+                if (regular) {
+                    prec = ci + sprec[fv];
+                    ++n_reg;
+                }
+                u64 rec = (u64)kk << lowbits;
+                if (keep) rec |= slab_low | (u64)((u32)lv1 * vmul + (u32)lx);
+                // ---- cofacet vertex below the top of s (whole rows of lanes: the columns holding the top vertices), or no
+                // cofacet of equal diameter: the facet test, the two small lists
+                if (__any_sync(RIPS_FULL_MASK, keep && !regular)) {
+                    bool is_irr = false, is_non = keep && !found;
+                    u64 irr_rec = 0;
+                    if (found && !regular) {
+                        int sv[M];
+                        sv[0] = lx;
+                        sv[1] = lv1;
+#pragma unroll
+                        for (int j = 2; j < M; ++j) sv[j] = v[j];
+                        int fseg = 0;
+#pragma unroll
+                        for (int j = 0; j < M; ++j) fseg += (sv[j] < fv) ? 1 : 0;
+                        if (s_is_youngest_facet<M, KT>(Kf, pitch, sv, key1, fv, fseg)) {
+                            irr_rec = (cofacet_index<M>(p.bt, sv, fv, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
+                            is_irr = true;
+                        } else
+                            is_non = true;
+                    }
+                    const u32 lt_mask = (1u << lane) - 1u;
+                    const u32 b_irr = __ballot_sync(RIPS_FULL_MASK, is_irr);
+                    if (b_irr) {
+                        u64 base = 0;
+                        if (lane == __ffs(b_irr) - 1)
+                            base = atomicAdd((unsigned long long*)(p.counters + S1C_IRREGULAR), (unsigned long long)__popc(b_irr));
+                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_irr) - 1) + __popc(b_irr & lt_mask);
+                        if (is_irr && base < p.irr_cap) p.irr_out[base] = irr_rec;
+                    }
+                    const u32 b_non = __ballot_sync(RIPS_FULL_MASK, is_non);
+                    if (b_non) {
+                        u64 base = 0;
+                        if (lane == __ffs(b_non) - 1)
+                            base = atomicAdd((unsigned long long*)(p.counters + S1C_NONAPP), (unsigned long long)__popc(b_non));
+                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_non) - 1) + __popc(b_non & lt_mask);
+                        if (is_non && base < p.non_cap) p.non_out[base] = rec;
+                    }
+                }
+                // ---- stores and the fused histograms
+                if (valid) {
+                    __stcs(p.cols_out + ci, rec);
+                    __stcs(p.pairs_out + ci, prec);
+#pragma unroll
+                    for (int r = 0; r < S1_MAX_FUSED; ++r)
+                        if (r < ncd) atomicAdd(&s_hist_cols[r][(kk >> (8 * r)) & 0xffu], 1u);
+                }
+#pragma unroll
+                for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
+                    if (r < npd) { // few distinct digits in a warp: aggregate
+                        const u32 dg = valid ? ((fvv >> (8 * r)) & 0xffu) : 0xffffffffu;
+                        const u32 peers = __match_any_sync(RIPS_FULL_MASK, dg);
+                        if (valid && lane == __ffs(peers) - 1) atomicAdd(&s_hist_pairs[r][dg], (u32)__popc(peers));
+                    }
+                }
+                // ---- next pair, 32 positions further in the order e = C(v1, 2) + x
+                lx += 32;
+                xo += pitch32;
+                while (lx >= lv1) { lx -= lv1; xo -= r1o; ++lv1; r1o += pitch; }
+            }
+            idx += (u64)seg;
+            rem -= seg;
+            e0 += seg;
+            if (e0 >= slab_len) { // next slab (colex successor of (v[M-1..2]))
+                e0 = 0;
+                if (M > 2) {
+#pragma unroll
+                    for (int j = 2; j < M; ++j) {
+                        v[j] += 1;
+                        if (j + 1 < M && v[j] == v[j + 1 < M ? j + 1 : j]) v[j] = j;
+                        else break;
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- counters and the fused histograms: once per block
+    n_over = warp_sum_u64(n_over);
+    n_clr = warp_sum_u32(n_clr);
+    n_reg = warp_sum_u32(n_reg);
+    if (lane == 0) {
+        if (n_over) atomicAdd((unsigned long long*)&p.counters[S1C_OVER], (unsigned long long)n_over);
+        if (n_clr) atomicAdd((unsigned long long*)&p.counters[S1C_CLEARED], (unsigned long long)n_clr);
+        if (n_reg) atomicAdd((unsigned long long*)&p.counters[S1C_REGULAR], (unsigned long long)n_reg);
+    }
+    __syncthreads();
+    for (int i = tid; i < ncd * 256; i += S1_THREADS) {
+        u32 c = (&s_hist_cols[0][0])[i];
+        if (c) atomicAdd((unsigned long long*)&p.fh_cols.hist[i], (unsigned long long)c);
+    }
+    for (int i = tid; i < npd * 256; i += S1_THREADS) {
+        u32 c = (&s_hist_pairs[0][0])[i];
+        if (c) atomicAdd((unsigned long long*)&p.fh_pairs.hist[i], (unsigned long long)c);
+    }
+}
+
 __global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, int shift, u64 mask)
 {
     i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
@@ -432,14 +719,9 @@ __global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i
     }
 }
 
-template <int M, typename KT>
-cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
+template <typename K>
+cudaError_t launch_persistent(K kern, const Stage1Params& p, size_t smem, cudaStream_t st)
 {
-    const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
-    const int k_in = (!p.compact && !p.count_only && kf_bytes <= S1_KF_SMEM_LIMIT) ? 1 : 0;
-    const size_t smem = (k_in ? kf_bytes : 0) +
-                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.stage_cap * 8 : 0);
-    auto kern = k_in ? enumerate_apparent_kernel<M, KT, true> : enumerate_apparent_kernel<M, KT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) return e;
     int per_sm = 1;
@@ -452,6 +734,24 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
     if (g > (i64)sms * per_sm) g = (i64)sms * per_sm;
     kern<<<(unsigned)g, S1_THREADS, smem, st>>>(p);
     return cudaGetLastError();
+}
+
+template <int M, typename KT>
+cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
+{
+    const size_t kf_bytes = (((size_t)p.n * p.pitch * sizeof(KT)) + 15) & ~(size_t)15;
+    const bool kf_fits = kf_bytes <= S1_KF_SMEM_LIMIT;
+    if (!p.compact && !p.count_only) {
+        // slot mode: the leaner kernel, if its tables fit (C(., M+1) and one row of U2 per warp)
+        const size_t tables = (size_t)p.n * 8 + (M > 2 ? (size_t)S1_WARPS * ((p.n + 7) & ~7) * sizeof(KT) : 0);
+        if (kf_fits && kf_bytes + tables <= 190 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, true>, p, kf_bytes + tables, st);
+        if (tables <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false>, p, tables, st);
+    }
+    const int k_in = (!p.compact && !p.count_only && kf_fits) ? 1 : 0;
+    const size_t smem = (k_in ? kf_bytes : 0) +
+                        ((p.compact && !p.count_only) ? (size_t)S1_WARPS * 2 * p.stage_cap * 8 : 0);
+    if (k_in) return launch_persistent(enumerate_apparent_kernel<M, KT, true>, p, smem, st);
+    return launch_persistent(enumerate_apparent_kernel<M, KT, false>, p, smem, st);
 }
 
 } // namespace
