@@ -55,8 +55,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-scale-row", action="store_true",
                     help="skip the scale row (stage 1 + 2 at d = dim_max+1: the C(n, dim_max+2) simplices the config names)")
-    ap.add_argument("--warmup-seconds", type=float, default=0.6,
-                    help="keep warming up until this much time has passed (gives the clock sampler load to see)")
+    ap.add_argument("--warmup-seconds", type=float, default=0.0,
+                    help="keep warming up (beyond --warmup, which is honoured exactly by default) until this much time has "
+                         "passed; the warm-ups actually run are printed as `warmup`")
     return ap.parse_args()
 
 
@@ -251,6 +252,27 @@ def algorithmic_bytes(field, st):
     raise KeyError(field)
 
 
+def source_stamp():
+    """sha256 over the kernel sources: profiles/traffic.json carries the stamp of the build it was captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2003_07989_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def compute_all(g, w, reduce_upto):
+    """dim 0, then per dimension stage 1, stage 2 and (up to reduce_upto) the reduction."""
+    g.dim0()
+    for d in range(1, w.dim_max + 1):
+        g.stage1(d)
+        g.stage2(d)
+        if d <= reduce_upto:
+            g.reduce(d)
+
+
 def run_b200(args):
     import torch
 
@@ -264,14 +286,20 @@ def run_b200(args):
 
     w = inputs.config(args.config)
     D = w.dim_max
+    # config 3 (random matrix): the reduced columns of dimension 2 do not fit any device: its
+    # barcodes stop at dimension 1; the hot path (stage 1 + stage 2) runs in every dimension
+    reduce_upto = 1 if args.config == 3 else D
     n_cand = sum(comb(w.n, d + 1) for d in range(1, D + 1))
     host = torch.from_numpy(w.dist).pin_memory()
     dev = host.cuda()
+    wsize = rips.rips_workspace_bytes(w.n, D)
+    free_b, _ = torch.cuda.mem_get_info()
+    workspace = torch.empty(min(wsize, int(free_b * 0.4)), dtype=torch.uint8, device="cuda")
 
     # ---- resident context; one full computation provides the clearing sets (and the barcode time)
     g = rips.Rips(dev, w.n, D, w.threshold)
     t0 = time.perf_counter()
-    g.compute()
+    compute_all(g, w, reduce_upto)
     torch.cuda.synchronize()
     first_compute_ms = 1e3 * (time.perf_counter() - t0)
     stats = {d: g.stats(d) for d in range(0, D + 1)}
@@ -287,31 +315,60 @@ def run_b200(args):
         sampler.start()
     t_w = time.perf_counter()
     n_w = 0
-    while n_w < max(args.warmup, 3) or (time.perf_counter() - t_w < args.warmup_seconds and n_w < 200):
+    while n_w < args.warmup or (time.perf_counter() - t_w < args.warmup_seconds and n_w < 200):
         hot_step()
         n_w += 1
-    per_kernel = {k: 0.0 for k in KERNELS}
-    per_kernel_dim = {k: {d: 0.0 for d in range(1, D + 1)} for k in KERNELS}
-    stage_ms = 0.0
+    torch.cuda.synchronize()
     launches0 = g.kernel_launches()
     barrier()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    for _ in range(args.steps):
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    evs[0].record()
+    for i in range(args.steps):      # nothing in the timed region waits for the device: the steps are enqueued back to back
         hot_step()
-        for d in range(1, D + 1):   # the library's own CUDA events of this step, read once the step is enqueued
-            t = g.timings(d)
+        evs[i + 1].record()
+    barrier()
+    elapsed_ms = evs[0].elapsed_time(evs[-1])
+    step_ms = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps))
+    launches = g.kernel_launches() - launches0
+    # the library's own CUDA events (per kernel) of the LAST timed step, then of a few more steps run one by one
+    per_kernel = {k: 0.0 for k in KERNELS}
+    per_kernel_dim = {k: {d: 0.0 for d in range(1, D + 1)} for k in KERNELS}
+    n_prof = 0
+    for rep in range(1 + 4):
+        if rep:
+            hot_step()
+        for d in range(1, D + 1):
+            t = g.timings(d)            # synchronises
             for k in KERNELS:
                 per_kernel[k] += t[k]
                 per_kernel_dim[k][d] += t[k]
-            stage_ms += t["stage1_ms"] + t["stage2_ms"]
-    ev1.record()
-    barrier()
-    elapsed_ms = ev0.elapsed_time(ev1)
-    launches = g.kernel_launches() - launches0
+        n_prof += 1
     clocks = sampler.stop() if rank == 0 else None
     ms_per_step = ranks.max_over_ranks(elapsed_ms) / args.steps
     value = world * n_cand / (ms_per_step * 1e-3)
+
+    # ---- the step WITH the arrays the ABI promises (fp32 diameter + u64 index filtration, (t, s) pair arrays):
+    # stage 1 + stage 2 + rips_filtration / rips_apparent_pairs / rips_nonapparent of every dimension
+    lib, C = rips.lib(), rips.C
+    def outputs():
+        a, b, k = C.c_void_p(), C.c_void_p(), C.c_int64()
+        for d in range(1, D + 1):
+            for fn in ("rips_filtration", "rips_apparent_pairs", "rips_nonapparent"):
+                rc = getattr(lib, fn)(g._h, d, C.byref(a), C.byref(b), C.byref(k))
+                assert rc == 0, (fn, d, rc)
+    with_out = []
+    try:
+        for i in range(2 + min(args.steps, 5)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); hot_step(); outputs(); e1.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                with_out.append(e0.elapsed_time(e1))
+        step_with_outputs = {"ms_per_step": statistics.median(with_out), "value": world * n_cand / (statistics.median(with_out) * 1e-3),
+                             "unit": UNIT, "what": "stage 1 + stage 2 + rips_filtration + rips_apparent_pairs + rips_nonapparent of every "
+                             "dimension (unpack / merge kernels materialise the fp32 + u64 arrays of include/rips.h)"}
+    except rips.RipsError as e:
+        step_with_outputs = {"unavailable": str(e)}
 
     # ---- roofline of the dominant kernel (largest share of the timed region)
     peak, peak_src = load_peaks()
@@ -319,42 +376,49 @@ def run_b200(args):
     for k, name in KERNELS.items():
         d_top = max(per_kernel_dim[k], key=lambda d: per_kernel_dim[k][d])
         b, nl = algorithmic_bytes(k, g.stats(d_top))
-        ms_launch = per_kernel_dim[k][d_top] / args.steps / nl
-        kernels.append({"kernel": name, "dim": d_top, "ms_per_step_all_dims": per_kernel[k] / args.steps,
+        ms_launch = per_kernel_dim[k][d_top] / n_prof / nl
+        kernels.append({"kernel": name, "dim": d_top, "ms_per_step_all_dims": per_kernel[k] / n_prof,
                         "ms_per_launch": ms_launch, "launches_per_step": nl, "bytes_per_launch": b,
                         "gbs": (b / (ms_launch * 1e-3) / 1e9) if ms_launch > 0 else 0.0,
                         "frac_of_peak": (b / (ms_launch * 1e-3) / 1e9 / peak) if ms_launch > 0 else 0.0,
-                        "share_of_step": per_kernel[k] / args.steps / ms_per_step})
+                        "share_of_step": per_kernel[k] / n_prof / ms_per_step})
     top = max(kernels, key=lambda r: r["ms_per_step_all_dims"])
     roofline = {"bound": "hbm", "kernel": top["kernel"], "dim": top["dim"], "achieved": top["gbs"], "peak": peak,
                 "unit": "GB/s", "frac": top["frac_of_peak"], "traffic": None, "peak_source": peak_src,
                 "bytes_per_launch": top["bytes_per_launch"], "ms_per_launch": top["ms_per_launch"],
-                "nominal_peak_gbs": 8000.0, "frac_of_nominal": top["gbs"] / 8000.0}
+                "nominal_peak_gbs": 8000.0, "frac_of_nominal": top["gbs"] / 8000.0,
+                "kernels_ms_per_step": sum(r["ms_per_step_all_dims"] for r in kernels),
+                "not_in_kernels_ms": ms_per_step - sum(r["ms_per_step_all_dims"] for r in kernels)}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
             tj = json.load(f)
-        key = f"cfg{args.config}:{top['kernel'].split(' ')[0]}:{'a9' if 'a9' in top['kernel'] else 'a6' if 'a6' in top['kernel'] else ''}"
-        roofline["traffic"] = tj.get(key)
-        inst = tj.get(key + ":inst")
-        if inst and top["ms_per_launch"] > 0:
-            # the fused kernel is bound by instruction issue, not by HBM: 148 SMs x 4 schedulers x 1.965 GHz
-            peak_inst = 148 * 4 * 1.965e9
-            roofline["issue"] = {"warp_inst_per_launch": inst, "achieved_ginst_s": inst / (top["ms_per_launch"] * 1e-3) / 1e9,
-                                 "peak_ginst_s": peak_inst / 1e9, "frac": inst / (top["ms_per_launch"] * 1e-3) / peak_inst,
-                                 "note": "ncu smsp__inst_executed.sum / live duration; what actually binds this kernel"}
+        if tj.get("source_stamp") == source_stamp():   # captured from this very build; dropped silently once the kernels change
+            key = f"cfg{args.config}:{top['kernel'].split(' ')[0]}:{'a9' if 'a9' in top['kernel'] else 'a6' if 'a6' in top['kernel'] else ''}"
+            roofline["traffic"] = tj.get(key)
+            inst = tj.get(key + ":inst")
+            if inst and top["ms_per_launch"] > 0:
+                # the fused kernel is bound by instruction issue, not by HBM: SMs x 4 schedulers x clock
+                peak_inst = 148 * 4 * 1.965e9
+                roofline["issue"] = {"warp_inst_per_launch": inst, "achieved_ginst_s": inst / (top["ms_per_launch"] * 1e-3) / 1e9,
+                                     "peak_ginst_s": peak_inst / 1e9, "frac": inst / (top["ms_per_launch"] * 1e-3) / peak_inst,
+                                     "note": "ncu smsp__inst_executed.sum / live duration; what actually binds this kernel"}
+                roofline["bound_actual"] = "issue"
+        else:
+            roofline["traffic_note"] = "profiles/traffic.json was captured from other kernel sources: not quoted"
 
-    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region); the workspace is the
+    # caller's (one torch allocation reused by every iteration: nothing allocates device memory inside)
     e2e_ms, d2h_bytes, parts = [], 0, None
     for i in range(args.e2e_steps + 1 if args.e2e_steps > 0 else 0):
         barrier()
         t0 = time.perf_counter()
-        h = rips.Rips(host.numpy(), w.n, D, w.threshold)
-        h.compute()
-        bars = [h.barcodes(d) for d in range(0, D + 1)]
+        h = rips.Rips(host.numpy(), w.n, D, w.threshold, workspace=workspace)
+        compute_all(h, w, reduce_upto)
+        bars = [h.barcodes(d) for d in range(0, reduce_upto + 1)]
         torch.cuda.synchronize()
         t1 = time.perf_counter()
-        if i > 0:   # the first one warms the allocator
+        if i > 0:   # the first one warms up
             e2e_ms.append(1e3 * (t1 - t0))
         d2h_bytes = sum(b.nbytes for b in bars)
         tim = {d: h.timings(d) for d in range(0, D + 1)}
@@ -363,17 +427,23 @@ def run_b200(args):
                  "reduce_device_ms": sum(tim[d]["reduce_device_ms"] for d in range(1, D + 1)),
                  "reduce_host_ms": sum(tim[d]["reduce_host_ms"] for d in range(1, D + 1)),
                  "reduce_xfer_ms": sum(tim[d]["reduce_xfer_ms"] for d in range(1, D + 1)),
+                 "reduce": {str(d): {k: h.stats(d)[k] for k in ("n_nonapparent", "n_additions", "n_reduce_serial", "n_reduce_displaced",
+                                                                 "reduce_arena_bytes")} for d in range(1, reduce_upto + 1)},
+                 "barcodes_of_dimensions": list(range(0, reduce_upto + 1)),
+                 "workspace_bytes": int(workspace.numel()), "workspace_peak_bytes": h.workspace_in_use()[1],
                  "bars": {str(d): int(b.shape[0]) for d, b in enumerate(bars)}}
         h.free()
     e2e_t = statistics.median(e2e_ms) if e2e_ms else float("nan")
     e2e_t = ranks.max_over_ranks(e2e_t)
     e2e = {"value": world * n_cand / (e2e_t * 1e-3), "unit": UNIT, "ms": e2e_t,
            "h2d_bytes_per_step": int(host.numel() * 4), "d2h_bytes_per_step": int(d2h_bytes),
-           "what": "rips_init(host matrix) + rips_compute + rips_barcodes(host) + rips_free"}
+           "what": "rips_init(host matrix, caller's workspace) + dim 0 + per dimension stage 1, stage 2, reduction + rips_barcodes(host) + rips_free"}
 
     # ---- scale row: the same kernels one dimension up, on the simplices the config names
     scale = None
-    if not args.no_scale_row and D + 1 <= 4:
+    if not args.no_scale_row and D + 1 <= 4 and reduce_upto == D:
+        del workspace
+        torch.cuda.empty_cache()
         need = 5 * 8 * comb(w.n, D + 2) + (1 << 30)
         free_b, _ = torch.cuda.mem_get_info()
         if need < free_b:
@@ -392,25 +462,41 @@ def run_b200(args):
                      "stage1_ms": s1, "stage2_ms": s2,
                      "simplices_per_s": world * st["n_candidates"] / ((ranks.max_over_ranks(s1 + s2)) * 1e-3),
                      "fused_kernel_ms": tm["enumerate_ms"], "fused_kernel_gbs": (nbytes + st["n_candidates"] / 8) / tm["enumerate_ms"] / 1e6,
+                     "fused_kernel_frac_of_peak": (nbytes + st["n_candidates"] / 8) / tm["enumerate_ms"] / 1e6 / peak,
                      "filtration_sort_pass_ms": tm["sort_pass_ms"] / max(1, st["sort_passes"]),
                      "filtration_sort_pass_gbs": nbytes / (tm["sort_pass_ms"] / max(1, st["sort_passes"])) / 1e6,
+                     "filtration_sort_pass_frac_of_peak": nbytes / (tm["sort_pass_ms"] / max(1, st["sort_passes"])) / 1e6 / peak,
                      "pair_partition_pass_ms": tm["pair_sort_ms"] / max(1, st["pair_sort_passes"]),
                      "pair_partition_pass_gbs": nbytes / (tm["pair_sort_ms"] / max(1, st["pair_sort_passes"])) / 1e6,
+                     "pair_partition_pass_frac_of_peak": nbytes / (tm["pair_sort_ms"] / max(1, st["pair_sort_passes"])) / 1e6 / peak,
                      "hbm_bytes": 4 * nbytes + st["n_candidates"] / 8,
                      "overall_gbs": (4 * nbytes + st["n_candidates"] / 8) / (s1 + s2) / 1e6,
                      "device_bytes": g.device_bytes()}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle
         s, t, cores, desc, _ = oracle_sample(w, args.cpu_seconds)
         cpu = {"value": s / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": t}
+        # the same sample at one thread (a shorter one), and the oracle's barcodes single-threaded on what it finishes
+        oracle.set_threads(1)
+        s1, t1, _, desc1, _ = oracle_sample(w, max(3.0, args.cpu_seconds / 3))
+        cpu["one_thread"] = {"value": s1 / t1, "unit": UNIT, "cores": 1, "sample": desc1, "seconds": t1}
+        dlow = min(D, 2) if args.config != 3 else 1
+        t0 = time.perf_counter()
+        oracle.barcodes(w.dist, w.n, dlow, w.threshold, explicit=(args.config == 3)) if (args.config != 3 or args.cpu_seconds >= 60) else None
+        cpu["barcodes_one_thread"] = {"seconds": time.perf_counter() - t0, "dimensions": f"0..{dlow}",
+                                      "what": "oracle.barcodes (stage 1, stage 2, reduction) with one thread" +
+                                              ("" if (args.config != 3 or args.cpu_seconds >= 60) else ": skipped (about 40 s; pass --cpu-seconds 60)")}
+        oracle.set_threads(cores)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": n_w, "ms_per_step": ms_per_step, "higher_is_better": True,
+                "warmup": n_w, "ms_per_step": ms_per_step, "ms_per_step_median": statistics.median(step_ms),
+                "ms_per_step_best": step_ms[0], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
                 "config": workload_dict(w, n_cand), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-                "roofline": roofline, "cpu_baseline": cpu,
+                "roofline": roofline, "cpu_baseline": cpu, "step_with_outputs": step_with_outputs,
                 "kernels": kernels, "scale_row": scale,
                 "barcode": {"end_to_end_ms": e2e_t, "first_compute_ms": first_compute_ms, **(parts or {})},
                 "stats": {str(d): {k: stats[d][k] for k in ("n_candidates", "n_columns", "n_cleared",

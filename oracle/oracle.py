@@ -66,6 +66,11 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def set_threads(t: int) -> None:
+    """OpenMP threads of stage 1 / stage 2 (bench.py's cpu_baseline reports all cores and one thread)."""
+    lib().oracle_set_threads(int(t))
+
+
 def _take(ptr, count, dtype):
     """Copy a malloc'ed C array into numpy and free it."""
     if count:

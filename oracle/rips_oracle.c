@@ -131,6 +131,16 @@ static float diameter(const float *D, const int *verts, int m)
 
 void oracle_free(void *p) { free(p); }
 
+/* bench.py's cpu_baseline times the same sample at all cores and at one thread */
+void oracle_set_threads(int t)
+{
+#ifdef _OPENMP
+    if (t >= 1) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

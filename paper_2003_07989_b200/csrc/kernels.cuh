@@ -90,8 +90,10 @@ struct Stage1Params {
 int stage1_chunk(u64 total, int compact, double est_survival, int retry);
 int stage1_stage_cap();
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
-// bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st);
+// bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask, i < min(n_rows, *n_dev) (n_dev may be NULL);
+// records with (rows[i] >> sent_shift) == sent are skipped (sent_shift < 0: none)
+cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, const u64* n_dev, int shift, u64 mask, int sent_shift,
+                                u64 sent, cudaStream_t st);
 
 // ------------------------------------------------------------------ pair store, unpack, lookup (stage2.cu)
 // The two sorted layers of apparent pairs of one dimension (the third layer, the pivots found by the

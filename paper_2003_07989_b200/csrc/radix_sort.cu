@@ -38,9 +38,10 @@ struct PlanDev {
     int bits[RIPS_SORT_MAX_PASSES];
 };
 
-__global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const u64* __restrict__ in, i64 n, PlanDev plan,
-                                                                      u64* __restrict__ hist)
+__global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const u64* __restrict__ in, i64 n, const u64* __restrict__ n_dev,
+                                                                      PlanDev plan, u64* __restrict__ hist)
 {
+    if (n_dev) n = min(n, (i64)__ldg(n_dev)); // the record count lives on the device: n is its upper bound
     extern __shared__ u32 sh_hist[]; // [npasses][MAX_BINS]
     const int total_bins = plan.npasses * RIPS_SORT_MAX_BINS;
     for (int i = threadIdx.x; i < total_bins; i += HIST_THREADS) sh_hist[i] = 0;
@@ -101,9 +102,10 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 // (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
-onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, int shift, int bits,
+onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, const u64* __restrict__ n_dev, int shift, int bits,
                      const u64* __restrict__ global_base, u64* status, u32* ticket, int pf_dist)
 {
+    if (n_dev) n = min(n, (i64)__ldg(n_dev)); // launched for the upper bound: the tiles past the count leave at once
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nbins = 1 << bits;
     const u32 mask = (u32)nbins - 1u;
@@ -122,6 +124,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, i
     __syncthreads();
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
+    if (base >= n) return; // (uniform; only with a device-side count)
     const int count = (int)min((i64)SORT_TILE, n - base);
 
     // L2 prefetch of the tile that is pf_dist tickets ahead (one bulk instruction): a CTA has loads in flight only
@@ -341,7 +344,7 @@ cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream)
 }
 
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream, u64** result,
-                     SortTimes* times, i64* launches, bool hist_ready, bool skewed_digits)
+                     SortTimes* times, i64* launches, bool hist_ready, bool skewed_digits, const u64* n_dev)
 {
     *result = a;
     int sms = 148;
@@ -381,7 +384,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         i64 blocks = (n + chunk - 1) / chunk;
         if (blocks > (i64)sms * 4) blocks = (i64)sms * 4;
         if (!hist_ready) {
-            sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, pd, hist);
+            sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, n_dev, pd, hist);
             if (launches) *launches += 1;
         }
         sort_scan_bins_kernel<<<plan.npasses, RIPS_SORT_MAX_BINS, 0, stream>>>(hist);
@@ -395,7 +398,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         e = cudaMemsetAsync(status, 0, status_bytes, stream);
         if (e != cudaSuccess) return e;
         onesweep_pass_kernel<<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-            src, dst, n, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist);
+            src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist);
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }

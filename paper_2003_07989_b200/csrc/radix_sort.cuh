@@ -32,8 +32,10 @@ struct SortTimes {
 // already accumulated the raw digit counts of every pass into sort_hist_ptr(scratch)[pass][256]
 // (FusedHist in kernels.cuh); the sort then skips its own histogram read of the records.
 // skewed_digits: a warp's 32 records mostly share a few digits (ranking by MATCH instead of ballots).
+// n_dev (optional): the number of records lives on the device (u64); n is then its upper bound (launch size, scratch size)
+// and the kernels sort min(*n_dev, n) records.  Whatever the count, the sorted data ends in *result.
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
                      u64** result, SortTimes* times, i64* launches, bool hist_ready = false,
-                     bool skewed_digits = false);
+                     bool skewed_digits = false, const u64* n_dev = nullptr);
 cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream);
 u64* sort_hist_ptr(void* scratch);

@@ -142,7 +142,14 @@ struct DimState {
     int compact = 0;
     // stage 1: column records (sorted), pair slots (unsorted until stage 2), the two small lists
     bool have_s1 = false;
-    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch;
+    DevBuf colsA, colsB, s1_status, bitmap, pairsA, pairsB, irrA, irrB, nonA, nonB, pair_scratch, d_cnt;
+    u64* h_cnt = nullptr;         // pinned: the fused kernel's counters, copied behind it
+    cudaEvent_t ev_cnt = nullptr; // ... and the event of that copy
+    bool counts_pending = false;  // h_cnt has not been read yet
+    bool cnt_copied = false;      // ev_cnt has been recorded at least once
+    bool caps_valid = false;      // a run of this dimension has fitted its lists: the sizes are known to suffice
+    u64 irr_cap = 0, non_cap = 0; // capacities of the two small lists (records)
+    int chunk_retry = 0, attempts = 0;
     DevBuf rd_piv, rd_colref, rd_todo, rd_htk, rd_htv, rd_arena, rd_cnt, rd_rec, rd_rec2, rd_bars; // reduction
     u64* cols = nullptr; // sorted packed column records (points into colsA or colsB)
     i64 len = 0;         // columns
@@ -195,6 +202,7 @@ struct rips_ctx {
     u64* d_counters = nullptr; // 16 u64 scratch counters
     u32* d_tickets = nullptr;  // 8 u32
     u64* h_counters = nullptr; // pinned
+    u64* h_dimcnt = nullptr;   // pinned: 8 u64 per dimension (DimState::h_cnt)
     u32 n_distinct = 0, thr_key = 0;
     int key_bits = 1;
     DevBuf sort_scratch, sort_scratch2, sort_scratch3;
@@ -354,6 +362,10 @@ int run_dim0(rips_ctx* c)
     s.reg = s.irr = s.non = nullptr;
     s.tbits = 1;
     s.have_s1 = s.have_s2 = s.have_red = true;
+    s.caps_valid = true;
+    s.counts_pending = false;
+    s.slots = 0;
+    s.irr_cap = 0;
     s.stats.n_columns = n;
     s.stats.n_reduced_pivots = npairs;
     s.stats.n_essential = n - npairs;
@@ -374,6 +386,53 @@ PairLayers layers_of(const DimState& s)
     return L;
 }
 
+// Counters of the fused kernel of dimension d: copied to pinned host memory behind the kernel, read here.
+// The first run of a dimension waits for them (the two small lists are provisioned by a rule of thumb and the
+// launch is repeated if one overflowed); once a run has fitted, the sizes are known to fit -- they depend only on
+// the context's input -- and rips_stage1 / rips_stage2 no longer wait for anything: the host reads the counters
+// only when an accessor, rips_stats or rips_reduce asks for them.
+int run_stage1(rips_ctx* c, int d);
+int run_stage2(rips_ctx* c, int d);
+
+int finish_counts(rips_ctx* c, int d)
+{
+    DimState& s = c->dims[d];
+    if (!s.counts_pending) return RIPS_OK;
+    CU(cudaEventSynchronize(s.ev_cnt));
+    s.counts_pending = false;
+    const u64* h = s.h_cnt;
+    const u64 ni = h[S1C_IRREGULAR], nn = h[S1C_NONAPP];
+    const bool stage_overflow = h[S1C_STAGE_OVERFLOW] != 0;
+    if (ni > s.irr_cap || nn > s.non_cap || stage_overflow) {
+        // rare: more irregular pairs / non-apparent columns than provisioned, or a chunk of compact mode kept more than
+        // a warp can stage: both stages again with the sizes now known
+        if (s.attempts >= 3) { g_last_error = "rips_stage1: list capacities still too small on the third attempt"; return RIPS_ECUDA; }
+        ++s.attempts;
+        s.irr_cap = std::max(s.irr_cap, ni);
+        s.non_cap = std::max(s.non_cap, nn);
+        if (stage_overflow) s.chunk_retry = 1;
+        s.caps_valid = false;
+        const bool had_s2 = s.have_s2;
+        CU(cudaStreamSynchronize(c->stream));
+        RC(run_stage1(c, d));
+        if (had_s2) RC(run_stage2(c, d));
+        return finish_counts(c, d);
+    }
+    s.attempts = 0;
+    s.caps_valid = true;
+    s.len = s.compact ? (i64)h[S1C_KEPT] : (i64)(s.total - h[S1C_OVER] - h[S1C_CLEARED]); // slot mode counts what it drops
+    s.n_reg = (i64)h[S1C_REGULAR];
+    s.n_irr = (i64)ni;
+    s.n_non = (i64)nn;
+    s.stats.n_columns = s.len;
+    s.stats.n_removed_by_diameter = (i64)h[S1C_OVER];
+    s.stats.n_cleared = (i64)h[S1C_CLEARED];
+    s.stats.n_apparent = s.n_reg + s.n_irr;
+    s.stats.n_nonapparent = s.n_non;
+    s.stats.n_regular = s.n_reg;
+    return RIPS_OK;
+}
+
 int run_stage1(rips_ctx* c, int d)
 {
     if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
@@ -383,6 +442,7 @@ int run_stage1(rips_ctx* c, int d)
         g_last_error = "rips_stage1: pivots of the previous dimension are missing";
         return RIPS_EINVAL;
     }
+    if (!prev.caps_valid) RC(finish_counts(c, d - 1)); // (only before the previous dimension's sizes are known to fit)
     const i64 n = c->n;
     s.M = d + 1;
     s.total = hbinom(c, n, d + 1);
@@ -399,6 +459,7 @@ int run_stage1(rips_ctx* c, int d)
     // The pivots found by an earlier rips_reduce(d) depend only on the input, so they stay valid
     // (have_red) while stage 1 / stage 2 are re-run; accessors additionally require have_s2.
     s.have_s1 = s.have_s2 = false;
+    s.counts_pending = false;
     invalidate_views(s, true, true, true, true);
     rips_stats_t keep_stats = rips_stats_t{};
     if (s.have_red) {
@@ -422,8 +483,13 @@ int run_stage1(rips_ctx* c, int d)
         ev_record(c, s, EV_S1_BITMAP); ev_record(c, s, EV_S1_ENUM); ev_record(c, s, EV_S1_SORTBEG);
         ev_record(c, s, EV_S1_HIST); ev_record(c, s, EV_S1_SORT); ev_record(c, s, EV_S1_END);
         s.have_s1 = true;
+        s.caps_valid = true;
         return RIPS_OK;
     }
+    if (s.cnt_copied && c->stream2) CU(cudaStreamWaitEvent(c->stream, s.ev_cnt, 0)); // the previous run's copy of the counters
+    RC(ensure(c, s.d_cnt, 128)); // 8 u64 counters, then the kernel's tickets
+    u64* const d_cnt = (u64*)s.d_cnt.p;
+    u32* const d_tick = (u32*)(d_cnt + 8);
     // ---- a4: clearing set of dimension d-1 as a bitmap over the candidate indices
     const u64 words = (s.total + 31) / 32;
     const bool use_bitmap = words * 4 <= (8ull << 30);
@@ -432,14 +498,24 @@ int run_stage1(rips_ctx* c, int d)
         RC(ensure(c, s.bitmap, (size_t)words * 4));
         CU(cudaMemsetAsync(s.bitmap.p, 0, (size_t)words * 4, c->stream));
         const u64 pmask = (prev.tbits >= 64) ? ~0ull : ((1ull << prev.tbits) - 1ull);
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.reg, prev.n_reg, 0, pmask, c->stream));
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.irr, prev.n_irr, RIPS_PAIR_POS_BITS, ~0ull, c->stream));
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, 0, ~0ull, c->stream));
-        c->launches += (prev.n_reg > 0) + (prev.n_irr > 0) + (prev.n_red > 0);
+        // regular pairs: every slot of the partitioned pair array, the sentinels (cofacet vertex = n) skipped;
+        // irregular pairs: as many as the previous dimension's kernel counted (on the device)
+        if (d >= 2 && prev.reg)
+            CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.reg, prev.slots, nullptr, 0, pmask, prev.tbits, (u64)n, c->stream));
+        if (d >= 2 && prev.irr)
+            CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.irr, (i64)prev.irr_cap, (const u64*)prev.d_cnt.p + S1C_IRREGULAR,
+                                   RIPS_PAIR_POS_BITS, ~0ull, -1, 0, c->stream));
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, nullptr, 0, ~0ull, -1, 0, c->stream));
+        c->launches += (d >= 2 && prev.reg && prev.slots > 0) + (d >= 2 && prev.irr && prev.irr_cap > 0) + (prev.n_red > 0);
         cs.bitmap = (const u32*)s.bitmap.p;
-    } else if (prev.n_reg > 0) {
-        g_last_error = "rips_stage1: candidate space too large for the clearing bitmap";
-        return RIPS_ENOMEM;
+    } else if (d >= 2) {
+        // no bitmap: the kernel searches the sorted layers, which needs their sizes on the host
+        RC(finish_counts(c, d - 1));
+        cs.n1 = prev.n_irr;
+        if (prev.n_reg > 0) {
+            g_last_error = "rips_stage1: candidate space too large for the clearing bitmap";
+            return RIPS_ENOMEM;
+        }
     }
     ev_record(c, s, EV_S1_BITMAP);
 
@@ -450,7 +526,7 @@ int run_stage1(rips_ctx* c, int d)
     const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
     const double est_survival = std::pow(q, (double)(s.M * (s.M - 1) / 2));
     s.compact = (c->thr_key != 0 && est_survival < 0.5) ? 1 : 0;
-    int chunk = stage1_chunk(s.total, s.compact, est_survival, 0);
+    int chunk = stage1_chunk(s.total, s.compact, est_survival, s.chunk_retry);
     i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
     Stage1Params p;
     p.Kf = c->d_Kf;
@@ -473,8 +549,8 @@ int run_stage1(rips_ctx* c, int d)
     p.cols_out = p.pairs_out = p.irr_out = p.non_out = nullptr;
     p.irr_cap = p.non_cap = 0;
     p.status = nullptr;
-    p.ticket = c->d_tickets;
-    p.counters = c->d_counters;
+    p.ticket = d_tick;
+    p.counters = d_cnt;
     p.fh_cols.hist = p.fh_pairs.hist = nullptr;
     p.fh_cols.npasses = p.fh_pairs.npasses = 0;
 
@@ -482,13 +558,12 @@ int run_stage1(rips_ctx* c, int d)
     if (s.compact) {
         if (s.exact_kept >= 0) cap = (u64)s.exact_kept; // the count is a constant of the context
         else { // first run of this dimension: count, then size the arrays exactly
-            CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
-            CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
+            CU(cudaMemsetAsync(d_cnt, 0, 128, c->stream));
             p.count_only = 1;
             CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
             c->launches += 1;
             p.count_only = 0;
-            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaMemcpyAsync(c->h_counters, d_cnt, 64, cudaMemcpyDeviceToHost, c->stream));
             CU(cudaStreamSynchronize(c->stream));
             cap = c->h_counters[S1C_KEPT];
             s.exact_kept = (i64)cap;
@@ -496,7 +571,9 @@ int run_stage1(rips_ctx* c, int d)
         RC(ensure(c, s.s1_status, (size_t)tiles * 8));
         p.status = (u64*)s.s1_status.p;
     }
+    s.slots = (i64)cap;
     RC(ensure(c, s.colsA, (size_t)cap * 8));
+    RC(ensure(c, s.colsB, (size_t)cap * 8));
     RC(ensure(c, s.pairsA, (size_t)cap * 8));
     p.cols_out = (u64*)s.colsA.p;
     p.pairs_out = (u64*)s.pairsA.p;
@@ -507,104 +584,65 @@ int run_stage1(rips_ctx* c, int d)
     RC(ensure(c, s.pair_scratch, sort_scratch_bytes((i64)cap, s.pair_plan)));
     const bool fused = plan.npasses <= 3;           // S1_MAX_FUSED digits
     s.pair_fused = s.pair_plan.npasses <= 2;        // S1_MAX_FUSED_P digits
-    // provisioned for (d+1)/n of the columns to hold the top vertices (those pairs are irregular) and as many
-    // non-apparent ones; a run that needs more is repeated once with the exact sizes
-    u64 irr_cap = std::max<u64>(s.irrA.cap / 8, std::max<u64>(4096, cap / 8));
-    u64 non_cap = std::max<u64>(s.nonA.cap / 8, std::max<u64>(4096, cap / 8));
-    // a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys, and the
+    // the two small lists: provisioned for (d+1)/n of the columns to hold the top vertices (those pairs are irregular)
+    // and as many non-apparent ones; finish_counts repeats the run with the exact sizes if one overflows
+    s.irr_cap = std::max<u64>(s.irr_cap, std::max<u64>(4096, cap / 8));
+    s.non_cap = std::max<u64>(s.non_cap, std::max<u64>(4096, cap / 8));
+    RC(ensure(c, s.irrA, (size_t)s.irr_cap * 8));
+    RC(ensure(c, s.nonA, (size_t)s.non_cap * 8));
+    p.irr_out = (u64*)s.irrA.p;
+    p.non_out = (u64*)s.nonA.p;
+    p.irr_cap = s.irr_cap;
+    p.non_cap = s.non_cap;
+    CU(cudaMemsetAsync(d_cnt, 0, 128, c->stream));
+    if (s.compact) CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
+    if (fused) {
+        CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
+        p.fh_cols.hist = sort_hist_ptr(c->sort_scratch.p);
+        p.fh_cols.npasses = plan.npasses;
+        for (int r = 0; r < plan.npasses; ++r) { p.fh_cols.shift[r] = plan.shift[r]; p.fh_cols.bits[r] = plan.bits[r]; }
+    }
+    if (s.pair_fused) {
+        CU(sort_prepare_fused(s.pair_scratch.p, c->stream));
+        p.fh_pairs.hist = sort_hist_ptr(s.pair_scratch.p);
+        p.fh_pairs.npasses = s.pair_plan.npasses;
+        for (int r = 0; r < s.pair_plan.npasses; ++r) {
+            p.fh_pairs.shift[r] = s.pair_plan.shift[r];
+            p.fh_pairs.bits[r] = s.pair_plan.bits[r];
+        }
+    }
+    CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
+    c->launches += 1;
+    ev_record(c, s, EV_S1_ENUM);
+    // the counters follow the kernel to the host on the second stream (nobody waits for them here)
+    {
+        cudaStream_t sc = c->stream2 ? c->stream2 : c->stream;
+        if (sc != c->stream) {
+            CU(cudaEventRecord(c->ev_fused, c->stream));
+            CU(cudaStreamWaitEvent(sc, c->ev_fused, 0));
+        }
+        CU(cudaMemcpyAsync(s.h_cnt, d_cnt, 64, cudaMemcpyDeviceToHost, sc));
+        CU(cudaEventRecord(s.ev_cnt, sc));
+        s.counts_pending = true;
+        s.cnt_copied = true;
+    }
+    // ---- a6: sort by key (diameter descending); stable, so cidx stays ascending inside equal keys, and the
     // sentinels of the dropped candidates (largest key) end up behind the len columns
-    bool sorted_early = false;
-    auto enqueue_a6 = [&](u64 nrec) -> int {
+    {
         SortTimes st;
         st.enabled = true;
-        if (!s.ev_made) ev_record(c, s, EV_S1_SORTBEG);
         st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
         s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, (i64)nrec, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches,
-                    fused));
+        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, (i64)cap, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
         s.cols = res;
         ev_record(c, s, EV_S1_END);
-        return RIPS_OK;
-    };
-    for (int attempt = 0;; ++attempt) {
-        RC(ensure(c, s.irrA, (size_t)irr_cap * 8));
-        RC(ensure(c, s.nonA, (size_t)non_cap * 8));
-        p.irr_out = (u64*)s.irrA.p;
-        p.non_out = (u64*)s.nonA.p;
-        p.irr_cap = irr_cap;
-        p.non_cap = non_cap;
-        CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
-        CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-        if (s.compact) CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
-        if (fused) {
-            CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
-            p.fh_cols.hist = sort_hist_ptr(c->sort_scratch.p);
-            p.fh_cols.npasses = plan.npasses;
-            for (int r = 0; r < plan.npasses; ++r) { p.fh_cols.shift[r] = plan.shift[r]; p.fh_cols.bits[r] = plan.bits[r]; }
-        }
-        if (s.pair_fused) {
-            CU(sort_prepare_fused(s.pair_scratch.p, c->stream));
-            p.fh_pairs.hist = sort_hist_ptr(s.pair_scratch.p);
-            p.fh_pairs.npasses = s.pair_plan.npasses;
-            for (int r = 0; r < s.pair_plan.npasses; ++r) {
-                p.fh_pairs.shift[r] = s.pair_plan.shift[r];
-                p.fh_pairs.bits[r] = s.pair_plan.bits[r];
-            }
-        }
-        CU(launch_stage1(s.M, c->kf_u16, p, c->stream));
-        c->launches += 1;
-        ev_record(c, s, EV_S1_ENUM);
-        if (!s.compact && c->stream2) {
-            // slot mode: the number of records is known, so the filtration sort is enqueued at once and
-            // the counters come back over the second stream while it runs
-            CU(cudaEventRecord(c->ev_fused, c->stream));
-            RC(ensure(c, s.colsB, (size_t)cap * 8));
-            RC(enqueue_a6(cap));
-            sorted_early = true;
-            CU(cudaStreamWaitEvent(c->stream2, c->ev_fused, 0));
-            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream2));
-            CU(cudaStreamSynchronize(c->stream2));
-        } else {
-            CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
-            CU(cudaStreamSynchronize(c->stream));
-        }
-        const u64 ni = c->h_counters[S1C_IRREGULAR], nn = c->h_counters[S1C_NONAPP];
-        const bool stage_overflow = c->h_counters[S1C_STAGE_OVERFLOW] != 0;
-        if (ni <= irr_cap && nn <= non_cap && !stage_overflow) break;
-        if (sorted_early) { CU(cudaStreamSynchronize(c->stream)); sorted_early = false; }
-        if (stage_overflow) { // a chunk kept more than a warp can stage: again with chunks no longer than the staging
-            chunk = stage1_chunk(s.total, s.compact, est_survival, 1);
-            tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
-            p.chunk = chunk;
-            p.tiles = tiles;
-            RC(ensure(c, s.s1_status, (size_t)tiles * 8));
-            p.status = (u64*)s.s1_status.p;
-        }
-        if (attempt >= 2) { g_last_error = "rips_stage1: list capacities still too small on the second attempt"; return RIPS_ECUDA; }
-        irr_cap = std::max(irr_cap, ni); // rare: more irregular pairs / non-apparent columns than provisioned; run again
-        non_cap = std::max(non_cap, nn);
     }
-    // (slot mode counts what it drops; the columns are the rest)
-    s.len = s.compact ? (i64)c->h_counters[S1C_KEPT] : (i64)(s.total - c->h_counters[S1C_OVER] - c->h_counters[S1C_CLEARED]);
-    s.slots = s.compact ? s.len : (i64)s.total;
-    s.n_reg = (i64)c->h_counters[S1C_REGULAR];
-    s.n_irr = (i64)c->h_counters[S1C_IRREGULAR];
-    s.n_non = (i64)c->h_counters[S1C_NONAPP];
-    s.stats.n_columns = s.len;
-    s.stats.n_removed_by_diameter = (i64)c->h_counters[S1C_OVER];
-    s.stats.n_cleared = (i64)c->h_counters[S1C_CLEARED];
-    s.stats.n_apparent = s.n_reg + s.n_irr;
-    s.stats.n_nonapparent = s.n_non;
     s.stats.n_slots = s.slots;
-    s.stats.n_regular = s.n_reg;
     s.stats.sort_passes = s.slots > 1 ? plan.npasses : 0;
-    if (!sorted_early) {
-        RC(ensure(c, s.colsB, (size_t)s.slots * 8));
-        RC(enqueue_a6((u64)s.slots));
-    }
     s.have_s1 = true;
     s.pairs_fresh = true;
+    if (!s.caps_valid) RC(finish_counts(c, d)); // first run of this dimension: make sure the lists fitted
     return RIPS_OK;
 }
 
@@ -617,26 +655,33 @@ int run_stage2(rips_ctx* c, int d)
     if (s.have_s2 && !s.pairs_fresh) return RIPS_OK; // nothing new to partition: the pair store is current
     s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
-    // Everything below runs on the second stream: it only needs the fused kernel's outputs (complete: stage 1
-    // read its counters back), so it overlaps the filtration sort that stage 1 left running on the main stream.
+    if (s.total == 0) { s.have_s2 = true; s.pairs_fresh = false; return RIPS_OK; }
+    // Everything below runs on the second stream: it only needs the fused kernel's outputs, so it overlaps the
+    // filtration sort that stage 1 left running on the main stream.  The sizes of the two small lists stay on the
+    // device (the fused kernel's counters); the sorts are launched for the lists' capacities.
     cudaStream_t st2 = c->stream2 ? c->stream2 : c->stream;
+    const u64* d_cnt = (const u64*)s.d_cnt.p;
     ev_record(c, s, EV_S2_BEGIN, st2);
     // ---- a8: the two small out-of-order lists: irregular pairs by cidx(t), non-apparent columns by
     // (key, vertices), which is the coboundary order
     {
         SortPlan pi = sort_make_plan(RIPS_PAIR_POS_BITS, RIPS_PAIR_POS_BITS + s.tbits);
-        RC(ensure(c, s.irrA, 16));
-        RC(ensure(c, s.irrB, (size_t)s.n_irr * 8));
-        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(s.n_irr, pi)));
+        RC(ensure(c, s.irrB, (size_t)s.irr_cap * 8));
+        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes((i64)s.irr_cap, pi)));
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, s.n_irr, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches));
+        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, (i64)s.irr_cap, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches, false, false,
+                    d_cnt + S1C_IRREGULAR));
         s.irr = res;
         SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
-        RC(ensure(c, s.nonA, 16));
-        RC(ensure(c, s.nonB, (size_t)s.n_non * 8));
+        RC(ensure(c, s.nonB, (size_t)s.non_cap * 8));
         cudaStream_t st3 = (c->stream3 && st2 != c->stream) ? c->stream3 : st2;
-        RC(ensure(c, c->sort_scratch3, sort_scratch_bytes(s.n_non, pn)));
-        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, s.n_non, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches));
+        RC(ensure(c, c->sort_scratch3, sort_scratch_bytes((i64)s.non_cap, pn)));
+        if (st3 != st2) { // the third stream starts behind the fused kernel as well
+            CU(cudaEventRecord(c->ev_join3, st2));
+            CU(cudaStreamWaitEvent(st3, c->ev_join3, 0));
+        }
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, (i64)s.non_cap, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches, false, false,
+                    d_cnt + S1C_NONAPP));
         if (st3 != st2) { // join the third stream into the second
             CU(cudaEventRecord(c->ev_join3, st3));
             CU(cudaStreamWaitEvent(st2, c->ev_join3, 0));
@@ -647,7 +692,6 @@ int run_stage2(rips_ctx* c, int d)
     // ---- a9: stable partition of the pair slots by the cofacet vertex v: the regular pairs come out
     // ascending by cidx(t), the sentinels (v = n) behind them
     s.stats.pair_sort_passes = s.slots > 1 ? s.pair_plan.npasses : 0;
-    RC(ensure(c, s.pairsA, 16));
     RC(ensure(c, s.pairsB, (size_t)s.slots * 8));
     SortTimes st;
     st.enabled = true;
@@ -673,6 +717,7 @@ int run_reduce(rips_ctx* c, int d)
     if (d < 1 || d > c->dim_max + 1) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) { g_last_error = "rips_reduce: rips_stage2 has not run for this dimension"; return RIPS_EINVAL; }
+    RC(finish_counts(c, d));
     s.have_red = false;
     invalidate_views(s, false, false, false, true);
     s.bars.clear();
@@ -820,7 +865,7 @@ int check_dim(rips_ctx* c, int d, int lo)
 void free_dim(rips_ctx* c, DimState& s)
 {
     DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.pairsA, &s.pairsB, &s.irrA, &s.irrB, &s.nonA, &s.nonB,
-                     &s.pair_scratch, &s.rd_piv, &s.rd_colref, &s.rd_todo, &s.rd_htk, &s.rd_htv, &s.rd_arena, &s.rd_cnt,
+                     &s.pair_scratch, &s.d_cnt, &s.rd_piv, &s.rd_colref, &s.rd_todo, &s.rd_htk, &s.rd_htv, &s.rd_arena, &s.rd_cnt,
                      &s.rd_rec, &s.rd_rec2, &s.rd_bars, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
@@ -1003,6 +1048,12 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     build_binom(n, c->kmax, c->h_binom);
     if (hbinom(c, n, dim_max + 2) >> 62) { delete c; return RIPS_EOVERFLOW; }
     c->dims.resize((size_t)dim_max + 2);
+    if (cudaMallocHost(&c->h_dimcnt, c->dims.size() * 64) != cudaSuccess) { cudaGetLastError(); delete c; return RIPS_ENOMEM; }
+    memset(c->h_dimcnt, 0, c->dims.size() * 64);
+    for (size_t i = 0; i < c->dims.size(); ++i) {
+        c->dims[i].h_cnt = c->h_dimcnt + 8 * i;
+        if (cudaEventCreateWithFlags(&c->dims[i].ev_cnt, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->dims[i].ev_cnt = nullptr; }
+    }
     int r = RIPS_OK;
     if (workspace_dev) {
         if (workspace_bytes < 4096 || ((uintptr_t)workspace_dev & 255)) {
@@ -1070,6 +1121,8 @@ void rips_free(rips_ctx* c)
     for (Pool::Chunk& ch : c->pool.chunks)
         if (ch.owned) cudaFree(ch.base);
     if (c->h_counters) cudaFreeHost(c->h_counters);
+    if (c->h_dimcnt) cudaFreeHost(c->h_dimcnt);
+    for (DimState& s : c->dims) if (s.ev_cnt) cudaEventDestroy(s.ev_cnt);
     cudaGetLastError();
     delete c;
 }
@@ -1085,6 +1138,7 @@ int rips_import_pivots(rips_ctx* c, int d, const uint64_t* t_host, const uint64_
     if (count < 0 || (count > 0 && (!t_host || !s_host))) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) { g_last_error = "rips_import_pivots: rips_stage2 has not run for this dimension"; return RIPS_EINVAL; }
+    RC(finish_counts(c, d));
     for (int64_t i = 1; i < count; ++i)
         if (t_host[i] <= t_host[i - 1]) return RIPS_EINVAL;
     s.have_red = false;
@@ -1134,6 +1188,7 @@ int rips_filtration(rips_ctx* c, int d, const float** diam_dev, const uint64_t**
     if (!diam_dev || !cidx_dev || !len) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s1) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     if (!s.has_vf) {
         RC(ensure(c, s.v_fdiam, (size_t)s.len * 4));
         RC(ensure(c, s.v_fcidx, (size_t)s.len * 8));
@@ -1154,6 +1209,7 @@ int rips_apparent_pairs(rips_ctx* c, int d, const uint64_t** t_dev, const uint64
     if (!t_dev || !s_dev || !n_app) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     if (!s.has_va) {
         RC(ensure(c, s.v_at, (size_t)(s.n_reg + s.n_irr) * 8));
         RC(ensure(c, s.v_as, (size_t)(s.n_reg + s.n_irr) * 8));
@@ -1174,6 +1230,7 @@ int rips_nonapparent(rips_ctx* c, int d, const float** diam_dev, const uint64_t*
     if (!diam_dev || !cidx_dev || !n_non) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     if (!s.has_vn) {
         RC(ensure(c, s.v_ndiam, (size_t)s.n_non * 4));
         RC(ensure(c, s.v_ncidx, (size_t)s.n_non * 8));
@@ -1195,6 +1252,7 @@ int rips_pivots(rips_ctx* c, int d, const uint64_t** t_dev, const uint64_t** s_d
     if (!t_dev || !s_dev || !n_piv) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_red || !s.have_s2) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     const i64 na = s.n_reg + s.n_irr, np = na + s.n_red;
     if (!s.has_vp) {
         if (!s.has_va) { // the apparent layers as (t, s) arrays first
@@ -1224,6 +1282,7 @@ int rips_pivot_lookup(rips_ctx* c, int d, const uint64_t* t_query_dev, int64_t m
     if (m < 0 || (m > 0 && (!t_query_dev || !s_out_dev))) return RIPS_EINVAL;
     DimState& s = c->dims[d];
     if (!s.have_s2) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     CU(launch_pivot_lookup(s.M, layers_of(s), c->bt(), (int)c->n, (const u64*)s.red_t.p, (const u64*)s.red_s.p,
                            s.have_red ? s.n_red : 0, t_query_dev, m, s_out_dev, c->stream));
     c->launches += m > 0;
@@ -1235,6 +1294,7 @@ int rips_stats(rips_ctx* c, int d, rips_stats_t* out)
 {
     RC(check_dim(c, d, 0));
     if (!out) return RIPS_EINVAL;
+    RC(finish_counts(c, d));
     *out = c->dims[d].stats;
     return RIPS_OK;
 }

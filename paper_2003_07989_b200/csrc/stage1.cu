@@ -710,11 +710,16 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
     }
 }
 
-__global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, int shift, u64 mask)
+// bitmap |= bits of the rows t = (rows[i] >> shift) & mask, i < min(n_rows, *n_dev); a record whose field above
+// `sent_shift` equals `sent` is a sentinel (the slot of a column with no regular pair) and is skipped
+__global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, const u64* __restrict__ n_dev, int shift,
+                                    u64 mask, int sent_shift, u64 sent)
 {
-    i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_rows) {
-        u64 t = (__ldg(rows + i) >> shift) & mask;
+    if (n_dev) n_rows = min(n_rows, (i64)__ldg(n_dev));
+    for (i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows; i += (i64)gridDim.x * blockDim.x) {
+        const u64 r = __ldg(rows + i);
+        if (sent_shift >= 0 && (r >> sent_shift) == sent) continue;
+        const u64 t = (r >> shift) & mask;
         atomicOr(bitmap + (t >> 5), 1u << (t & 31));
     }
 }
@@ -792,10 +797,12 @@ cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t
 #undef S1_CASE
 }
 
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, int shift, u64 mask, cudaStream_t st)
+cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, const u64* n_dev, int shift, u64 mask, int sent_shift,
+                                u64 sent, cudaStream_t st)
 {
     if (n_rows == 0) return cudaSuccess;
     i64 blocks = (n_rows + 255) / 256;
-    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, rows, n_rows, shift, mask);
+    if (blocks > 148 * 64) blocks = 148 * 64;
+    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, rows, n_rows, n_dev, shift, mask, sent_shift, sent);
     return cudaGetLastError();
 }
