@@ -475,8 +475,8 @@ int run_stage1(rips_ctx* c, int d)
     s.stats.n_candidates = (i64)s.total;
     s.stats.key_bits = c->key_bits;
     s.stats.index_bits = s.lowbits;
-    s.len = s.slots = 0;
-    s.n_reg = s.n_irr = s.n_non = 0;
+    if (!s.caps_valid) { s.len = 0; s.n_reg = s.n_irr = s.n_non = 0; } // (else: constants of the context, kept for sizing the launches)
+    s.slots = 0;
     s.cols = s.reg = s.irr = s.non = nullptr;
     ev_record(c, s, EV_S1_BEGIN);
     if (s.total == 0) {
@@ -656,12 +656,36 @@ int run_stage2(rips_ctx* c, int d)
     s.have_s2 = false;
     invalidate_views(s, false, true, true, true);
     if (s.total == 0) { s.have_s2 = true; s.pairs_fresh = false; return RIPS_OK; }
-    // Everything below runs on the second stream: it only needs the fused kernel's outputs, so it overlaps the
-    // filtration sort that stage 1 left running on the main stream.  The sizes of the two small lists stay on the
-    // device (the fused kernel's counters); the sorts are launched for the lists' capacities.
+    // Everything below runs beside the filtration sort that stage 1 left running on the main stream: it only needs the
+    // fused kernel's outputs.  Second stream: the pair partition (the large one: it shares the HBM with the
+    // filtration sort), then the irregular pairs; third stream: the non-apparent columns (short chains of small
+    // passes, bound by launch latency, so they run beside the large ones instead of in front of them).  The sizes of
+    // the two small lists stay on the device (the fused kernel's counters); once a run of this dimension has been
+    // checked they are constants of the context and the launches are sized by them, before that by the capacities.
     cudaStream_t st2 = c->stream2 ? c->stream2 : c->stream;
+    cudaStream_t st3 = (c->stream3 && st2 != c->stream) ? c->stream3 : st2;
     const u64* d_cnt = (const u64*)s.d_cnt.p;
+    const i64 irr_n = s.caps_valid ? std::max<i64>(s.n_irr, 1) : (i64)s.irr_cap;
+    const i64 non_n = s.caps_valid ? std::max<i64>(s.n_non, 1) : (i64)s.non_cap;
     ev_record(c, s, EV_S2_BEGIN, st2);
+    if (st3 != st2) { // the third stream starts behind the fused kernel as well
+        CU(cudaEventRecord(c->ev_join3, st2));
+        CU(cudaStreamWaitEvent(st3, c->ev_join3, 0));
+    }
+    // ---- a9: stable partition of the pair slots by the cofacet vertex v: the regular pairs come out
+    // ascending by cidx(t), the sentinels (v = n) behind them
+    {
+        s.stats.pair_sort_passes = s.slots > 1 ? s.pair_plan.npasses : 0;
+        RC(ensure(c, s.pairsB, (size_t)s.slots * 8));
+        SortTimes st;
+        st.enabled = true;
+        st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
+        s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
+        u64* res = nullptr;
+        CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, st2, &res, &st,
+                    &c->launches, s.pair_fused, true));
+        s.reg = res;
+    }
     // ---- a8: the two small out-of-order lists: irregular pairs by cidx(t), non-apparent columns by
     // (key, vertices), which is the coboundary order
     {
@@ -669,18 +693,13 @@ int run_stage2(rips_ctx* c, int d)
         RC(ensure(c, s.irrB, (size_t)s.irr_cap * 8));
         RC(ensure(c, c->sort_scratch2, sort_scratch_bytes((i64)s.irr_cap, pi)));
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, (i64)s.irr_cap, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches, false, false,
+        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, irr_n, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches, false, false,
                     d_cnt + S1C_IRREGULAR));
         s.irr = res;
         SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
         RC(ensure(c, s.nonB, (size_t)s.non_cap * 8));
-        cudaStream_t st3 = (c->stream3 && st2 != c->stream) ? c->stream3 : st2;
         RC(ensure(c, c->sort_scratch3, sort_scratch_bytes((i64)s.non_cap, pn)));
-        if (st3 != st2) { // the third stream starts behind the fused kernel as well
-            CU(cudaEventRecord(c->ev_join3, st2));
-            CU(cudaStreamWaitEvent(st3, c->ev_join3, 0));
-        }
-        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, (i64)s.non_cap, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches, false, false,
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, non_n, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches, false, false,
                     d_cnt + S1C_NONAPP));
         if (st3 != st2) { // join the third stream into the second
             CU(cudaEventRecord(c->ev_join3, st3));
@@ -689,18 +708,6 @@ int run_stage2(rips_ctx* c, int d)
         s.non = res;
     }
     ev_record(c, s, EV_S2_APP, st2);
-    // ---- a9: stable partition of the pair slots by the cofacet vertex v: the regular pairs come out
-    // ascending by cidx(t), the sentinels (v = n) behind them
-    s.stats.pair_sort_passes = s.slots > 1 ? s.pair_plan.npasses : 0;
-    RC(ensure(c, s.pairsB, (size_t)s.slots * 8));
-    SortTimes st;
-    st.enabled = true;
-    st.ev[0] = s.ev[EV_S2_SORTBEG]; st.ev[1] = s.ev[EV_S2_HIST]; st.ev[2] = s.ev[EV_S2_SORT];
-    s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
-    u64* res = nullptr;
-    CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, st2, &res, &st,
-                &c->launches, s.pair_fused, true));
-    s.reg = res;
     ev_record(c, s, EV_S2_END, st2);
     if (st2 != c->stream) { // join: whatever follows on the main stream sees stage 2's results
         CU(cudaEventRecord(c->ev_join, st2));
