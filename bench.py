@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k-1]; 2 is the one the metric is quoted on")
+    ap.add_argument("--n", type=int, default=None, help="point count override (config 6, the second workload of PAPER.md:719-729: n = 1000 .. 20000)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
@@ -118,7 +119,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from paper_2003_07989_b200 import inputs
-    w = inputs.config(args.config)
+    w = inputs.config(args.config, args.n)
     n_cand = sum(comb(w.n, d + 1) for d in range(1, w.dim_max + 1))
     per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
@@ -284,11 +285,13 @@ def run_b200(args):
     from paper_2003_07989_b200 import inputs, rips
     rips.lib()
 
-    w = inputs.config(args.config)
+    w = inputs.config(args.config, args.n)
     D = w.dim_max
     # config 3 (random matrix): the reduced columns of dimension 2 do not fit any device: its
     # barcodes stop at dimension 1; the hot path (stage 1 + stage 2) runs in every dimension
     reduce_upto = 1 if args.config == 3 else D
+    if args.config == 6:      # the second workload measures the apparent fraction of dimension 1: stage 1 + stage 2 only
+        reduce_upto = 0
     n_cand = sum(comb(w.n, d + 1) for d in range(1, D + 1))
     host = torch.from_numpy(w.dist).pin_memory()
     dev = host.cuda()
@@ -504,6 +507,12 @@ def run_b200(args):
                                                             "n_nonapparent", "n_slots", "sort_passes",
                                                             "pair_sort_passes", "key_bits", "index_bits")} for d in range(1, D + 1)},
                 "device_bytes": g.device_bytes(), "parallelism": "replicas" if world > 1 else "single"}
+        if args.config == 6:
+            import math
+            closed = 1 - (math.sqrt(math.pi) / 2) * math.exp(math.lgamma(w.n - 1) - math.lgamma(w.n - 0.5))
+            line["apparent_fraction"] = {"measured": stats[1]["n_apparent"] / comb(w.n, 2), "closed_form": closed,
+                                         "paper": {"10000": 0.991127743, "20000": 0.993733522}.get(str(w.n)),
+                                         "what": "apparent pairs of dimension 1 / C(n,2) (PAPER.md:723, :729)"}
         print(json.dumps(line))
     g.free()
     ranks.close()

@@ -352,9 +352,15 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         int dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
-    if (times && times->enabled) cudaEventRecord(times->ev[0], stream);
+    auto rec = [&](int i) {
+        if (!times || !times->enabled) return;
+        if (times->external) cudaEventRecordWithFlags(times->ev[i], stream, cudaEventRecordExternal);
+        else cudaEventRecord(times->ev[i], stream);
+    };
+    rec(0);
     if (n <= 1) {
-        if (times && times->enabled) { cudaEventRecord(times->ev[1], stream); cudaEventRecord(times->ev[2], stream); }
+        rec(1);
+        rec(2);
         return cudaSuccess;
     }
     {   // per call (cheap) rather than once per process: the attribute is per device
@@ -390,7 +396,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         sort_scan_bins_kernel<<<plan.npasses, RIPS_SORT_MAX_BINS, 0, stream>>>(hist);
         if (launches) *launches += 1;
     }
-    if (times && times->enabled) cudaEventRecord(times->ev[1], stream);
+    rec(1);
     u64* src = a;
     u64* dst = b;
     for (int p = 0; p < plan.npasses; ++p) {
@@ -402,7 +408,7 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }
-    if (times && times->enabled) cudaEventRecord(times->ev[2], stream);
+    rec(2);
     *result = src;
     return cudaGetLastError();
 }

@@ -23,6 +23,7 @@ size_t sort_scratch_bytes(i64 n, const SortPlan& plan);
 struct SortTimes {
     cudaEvent_t ev[3]; // optional: [0] before histogram, [1] after histogram, [2] after the last pass
     bool enabled;
+    bool external = false; // the stream is being captured: record the events as external event nodes
 };
 
 // Stable LSD sort of n u64 records by the plan's digits, ascending.  `a` holds the input, `b` is the

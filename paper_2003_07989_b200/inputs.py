@@ -142,7 +142,24 @@ def config(k: int, n: int | None = None) -> Workload:
         low = euclidean_lower(gaussian_points(n, 8, 4))
         return Workload(f"cfg5_gauss8_encl_n{n}", n, 2, enclosing_radius(low, n), low,
                         "standard Gaussian in R^8, seed 4, threshold = enclosing radius")
+    if k == 6:
+        return second_workload(n or 5000)
     raise ValueError(f"no config {k}")
+
+
+def second_workload(n: int, seed: int = 7) -> Workload:
+    """The experiment of PAPER.md:719-729 (section 6.6, Fig. 13): dimension-1 apparent pairs of a random distance
+    matrix with no triangle inequality.  n <= 5792: a uniformly random permutation of 1..n(n-1)/2 (exact in fp32);
+    above that the integers are no longer exact in fp32, so i.i.d. Uniform(0,1) fp32 entries are used (a few tied
+    values among 10^8: the closed form of the apparent fraction assumes none and is off by far less than its own
+    sampling noise)."""
+    if n <= 5792:
+        low = permutation_matrix_lower(n, seed)
+        note = "uniformly random permutation matrix (PAPER.md:719)"
+    else:
+        low = random_matrix_lower(n, seed)
+        note = "i.i.d. U(0,1) fp32 distance matrix (permutation values are not exact in fp32 beyond n = 5792)"
+    return Workload(f"sec66_randmat_n{n}", n, 1, INF, low, note + ", dimension 1 only, full complex")
 
 
 def n_choose_k(n: int, k: int) -> int:

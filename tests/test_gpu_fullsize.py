@@ -32,21 +32,17 @@ def R():
     return rips
 
 
-def oracle_clearing_sets(w, reduce):
-    """Pivot rows of every dimension below the top one, from the oracle's own pipeline.  reduce=False:
-    only the apparent pairs of the lower dimensions clear (the serial reduction of config 3's random
-    matrices is a "difficult" one, and far outside a test's time at n = 400; the kernels
-    under test take the clearing set as an input, and both sides get the same one)."""
+def oracle_clearing_sets(w, explicit=False):
+    """Pivot rows of every dimension below the top one, from the oracle's own pipeline (the TRUE clearing sets:
+    apparent pairs united with the pivots of the reduction).  explicit: the oracle's second reduction (Algorithm 1
+    on the explicit matrix), for config 3's random matrix, whose reduced columns fill in."""
     z = oracle.dim0(w.dist, w.n, w.threshold)
     cleared = {1: z["t"]}
     for d in range(1, w.dim_max):
         fd, fc, _ = oracle.stage1(w.dist, w.n, d, w.threshold, cleared[d])
         s2 = oracle.stage2(w.dist, w.n, d, fd, fc)
-        if reduce:
-            red = oracle.reduce_columns(w.dist, w.n, d, w.threshold, s2["non_cidx"], s2["app_t"], s2["app_s"])
-            cleared[d + 1] = np.sort(np.concatenate([s2["app_t"], red["t"]]))
-        else:
-            cleared[d + 1] = s2["app_t"]
+        red = oracle.reduce_columns(w.dist, w.n, d, w.threshold, s2["non_cidx"], s2["app_t"], s2["app_s"], explicit=explicit)
+        cleared[d + 1] = np.sort(np.concatenate([s2["app_t"], red["t"]]))
     return cleared
 
 
@@ -58,24 +54,21 @@ def slices_of(total):
     return [(0, SLICE), (mid, mid + SLICE), (total - SLICE, total)]
 
 
-def check_top_dimension(R, w, reduce=True):
+def check_top_dimension(R, w, explicit=False):
     import torch
     D, n = w.dim_max, w.n
-    cleared = oracle_clearing_sets(w, reduce)
+    cleared = oracle_clearing_sets(w, explicit)
     with R.Rips(w.dist, n, D, w.threshold) as g:
         g.dim0()
         for d in range(1, D):
             g.stage1(d); g.stage2(d)
-            if reduce:
-                g.reduce(d)
-            else:
-                g.import_pivots(d, [], [])
-        g.stage1(D); g.stage2(D)          # the reduction of the top dimension is not the hot path
+            g.reduce(d)
+        g.stage1(D); g.stage2(D)          # (the barcodes of the top dimension: test_full_size_barcodes)
         st = g.stats(D)
         total = comb(n, D + 1)
         assert st["n_candidates"] == total
         assert st["n_columns"] + st["n_removed_by_diameter"] + st["n_cleared"] == total
-        if w.threshold == inf and reduce:
+        if w.threshold == inf:
             assert st["n_columns"] == comb(n - 1, D + 1) and st["n_removed_by_diameter"] == 0
         assert st["n_apparent"] + st["n_nonapparent"] == st["n_columns"]
         fd, fc = g.filtration(D)
@@ -126,7 +119,69 @@ def check_top_dimension(R, w, reduce=True):
 
 @pytest.mark.parametrize("k", [2, 3, 4, 5])
 def test_full_size_sampled(R, k):
-    check_top_dimension(R, inputs.config(k), reduce=(k != 3))
+    check_top_dimension(R, inputs.config(k), explicit=(k == 3))
+
+
+def _compare_dimension(g, o, d, tag):
+    pt, ps = g.pivots(d)
+    assert np.array_equal(pt.cpu().numpy().astype(np.uint64), o[d]["pivot_t"]), tag
+    assert np.array_equal(ps.cpu().numpy().astype(np.uint64), o[d]["pivot_s"]), tag
+    assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32)), tag
+    if d == 0:
+        return
+    fd, fc = g.filtration(d)
+    assert np.array_equal(fc.cpu().numpy().astype(np.uint64), o[d]["filt_cidx"]), tag
+    assert np.array_equal(fd.cpu().numpy().view(np.uint32), o[d]["filt_diam"].view(np.uint32)), tag
+    at, as_ = g.apparent_pairs(d)
+    assert np.array_equal(at.cpu().numpy().astype(np.uint64), o[d]["app_t"]), tag
+    assert np.array_equal(as_.cpu().numpy().astype(np.uint64), o[d]["app_s"]), tag
+    nd, nc = g.nonapparent(d)
+    assert np.array_equal(nc.cpu().numpy().astype(np.uint64), o[d]["non_cidx"]), tag
+    st = g.stats(d)
+    assert st["n_essential"] == o[d]["essential"].size and st["n_reduced_pivots"] == o[d]["red_t"].size, tag
+
+
+@pytest.mark.parametrize("k", [2, 4, 5])
+def test_full_size_barcodes(R, k):
+    """BASELINE.json configs 2, 4, 5 at full size through rips_compute: EVERY array of EVERY dimension -- filtration,
+    apparent pairs, non-apparent columns, pivots (apparent united with the device reduction's), bars -- element by
+    element against the oracle's whole pipeline (oracle.barcodes: Algorithms 7-8, 3, and the reduction).  Config 2's
+    dimension 3 costs the oracle about a minute (54.9 million candidates, 142,819 columns to reduce)."""
+    w = inputs.config(k)
+    o = oracle.barcodes(w.dist, w.n, w.dim_max, w.threshold)
+    with R.Rips(w.dist, w.n, w.dim_max, w.threshold) as g:
+        g.compute()
+        for d in range(0, w.dim_max + 1):
+            _compare_dimension(g, o, d, f"{w.name} d={d}")
+        if w.threshold == inf:   # P9: every column of a full complex gets a pivot, no essential class above dimension 0
+            for d in range(1, w.dim_max + 1):
+                assert g.stats(d)["n_essential"] == 0 and g.pivots(d)[0].numel() == comb(w.n - 1, d + 1)
+
+
+def test_config3_dimension1_barcodes_and_dimension2_columns(R):
+    """Config 3 (400-point random matrix).  Dimension 1 completely: the device reduction (3,118 columns, ~1.5e5
+    additions, reduced columns of up to 10^6 entries) against the oracle's explicit reduction.  Dimension 2: stage 1
+    and stage 2 with the TRUE clearing set (the pivots of dimension 1), checked by test_full_size_sampled on slices
+    and here by the properties that hold at any size; its reduction is out of reach of any sparse Z/2 reduction at
+    n = 400 (~10^13 entries to add), so it has no barcodes to compare."""
+    import torch
+    w = inputs.config(3)
+    o = oracle.barcodes(w.dist, w.n, 1, w.threshold, explicit=True)
+    with R.Rips(w.dist, w.n, 2, w.threshold) as g:
+        g.dim0()
+        g.stage1(1); g.stage2(1); g.reduce(1)
+        for d in (0, 1):
+            _compare_dimension(g, o, d, f"{w.name} d={d}")
+        assert g.pivots(1)[0].numel() == comb(w.n - 1, 2) and g.stats(1)["n_essential"] == 0
+        g.stage1(2); g.stage2(2)
+        st = g.stats(2)
+        assert st["n_cleared"] == comb(w.n - 1, 2) and st["n_columns"] == comb(w.n - 1, 3)      # P9
+        assert st["n_apparent"] + st["n_nonapparent"] == st["n_columns"]
+        at, as_ = g.apparent_pairs(2)
+        assert bool((at[1:] > at[:-1]).all()) and torch.unique(as_).numel() == as_.numel()     # all t, all s distinct
+        idx = torch.linspace(0, at.numel() - 1, 200).long()
+        for t, s_ in zip(at[idx].tolist(), as_[idx].tolist()):                                  # zero persistence (PAPER.md:260)
+            assert oracle.diameter(w.dist, t, 4, w.n) == oracle.diameter(w.dist, s_, 3, w.n)
 
 
 def test_config2_lower_dimensions_complete(R):
@@ -146,15 +201,16 @@ def test_config2_lower_dimensions_complete(R):
             assert np.array_equal(g.barcodes(d).view(np.uint32), o[d]["bars"].reshape(-1, 2).view(np.uint32))
 
 
-def test_second_workload_dim1_random_permutation_matrix(R):
-    """SURVEY.md 8(f) item 4, the experiment of PAPER.md:719-729: dimension-1 apparent pairs of a uniformly
-    random permutation matrix.  (a) the apparent fraction against the closed form behind the paper's printed
-    means (pin P11; the paper reports a very low variance); (b) on a slice of the edges, the exact arrays
-    against the oracle."""
+@pytest.mark.parametrize("n", [1000, 3000, 5792, 10000])
+def test_second_workload_dim1_random_matrix(R, n):
+    """SURVEY.md 8(f) item 4, the experiment of PAPER.md:719-729 as a sweep: dimension-1 apparent pairs of a random
+    matrix without triangle inequality (a random permutation of 1..C(n,2) up to n = 5792, i.i.d. uniform fp32 above).
+    (a) the apparent fraction against the closed form behind the paper's printed means (pin P11; the paper reports a
+    very low variance); (b) on slices of the edges, the exact arrays against the oracle."""
     import math
     import torch
-    n = 3000
-    low = inputs.permutation_matrix_lower(n, 7)
+    w = inputs.second_workload(n)
+    low = w.dist
     E = n * (n - 1) // 2
     with R.Rips(torch.from_numpy(low).cuda(), n, 1) as g:
         g.dim0()
@@ -163,20 +219,24 @@ def test_second_workload_dim1_random_permutation_matrix(R):
         st = g.stats(1)
         assert st["n_candidates"] == E and st["n_cleared"] == n - 1 and st["n_columns"] == E - (n - 1)
         closed = 1 - (math.sqrt(math.pi) / 2) * math.exp(math.lgamma(n - 1) - math.lgamma(n - 0.5))
-        assert abs(st["n_apparent"] / E - closed) < 1e-3
+        assert abs(st["n_apparent"] / E - closed) < (3e-3 if n <= 1000 else 1e-3)
         z = oracle.dim0(low, n)
-        lo, hi = E // 2, E // 2 + 20000
-        od, oc, _ = oracle.stage1(low, n, 1, inf, z["t"], lo, hi, sort=False)
-        s2 = oracle.stage2(low, n, 1, od, oc)
+        pt, ps = g.pivots(0)
+        assert np.array_equal(pt.cpu().numpy().astype(np.uint64), z["t"])
         at, as_ = g.apparent_pairs(1)
-        m = (as_ >= lo) & (as_ < hi)
-        gs, order = torch.sort(as_[m])
-        o_order = np.argsort(s2["app_s"], kind="stable")
-        assert np.array_equal(gs.cpu().numpy().astype(np.uint64), s2["app_s"][o_order])
-        assert np.array_equal(at[m][order].cpu().numpy().astype(np.uint64), s2["app_t"][o_order])
         nd, nc = g.nonapparent(1)
-        m = (nc >= lo) & (nc < hi)
-        assert np.array_equal(torch.sort(nc[m])[0].cpu().numpy().astype(np.uint64), np.sort(s2["non_cidx"]))
+        assert bool((at[1:] > at[:-1]).all())
+        for lo in (0, E // 2, E - 20000):
+            hi = lo + 20000
+            od, oc, _ = oracle.stage1(low, n, 1, inf, z["t"], lo, hi, sort=False)
+            s2 = oracle.stage2(low, n, 1, od, oc)
+            m = (as_ >= lo) & (as_ < hi)
+            gs, order = torch.sort(as_[m])
+            o_order = np.argsort(s2["app_s"], kind="stable")
+            assert np.array_equal(gs.cpu().numpy().astype(np.uint64), s2["app_s"][o_order])
+            assert np.array_equal(at[m][order].cpu().numpy().astype(np.uint64), s2["app_t"][o_order])
+            m = (nc >= lo) & (nc < hi)
+            assert np.array_equal(torch.sort(nc[m])[0].cpu().numpy().astype(np.uint64), np.sort(s2["non_cidx"]))
 
 
 def test_compact_mode_with_dense_runs(R):
