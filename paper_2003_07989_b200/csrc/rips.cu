@@ -746,7 +746,10 @@ int run_reduce(rips_ctx* c, int d)
         const double t0 = now_ms();
         const i64 nn = s.n_non;
         const int jbits = bits_for((u64)(nn - 1));
-        if (s.tbits + jbits > 64) { g_last_error = "rips_reduce: (row, column) records do not fit 64 bits"; return RIPS_EOVERFLOW; }
+        if (s.tbits + jbits > 64 || c->key_bits + s.tbits > 63) {
+            g_last_error = "rips_reduce: (key, row) entries or (row, column) records do not fit 64 bits";
+            return RIPS_EOVERFLOW;
+        }
         u32 ht_cap = 1024;
         while ((u64)ht_cap < 2ull * (u64)nn) ht_cap <<= 1;
         const int sort_cap = reduce_sort_cap((int)c->n);
@@ -1114,7 +1117,8 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
         // the widest record of the requested dimensions must fit 64 bits
         int lb = (dim_max + 1) * c->vbits;
         int tb = bits_for(hbinom(c, n, dim_max + 2));
-        if ((dim_max >= 1 && c->key_bits + lb > 64) || c->key_bits + tb > 64 || bits_for((u64)n) + tb > 64)
+        // (the reduction's entries, key and row index in one word, are checked by rips_reduce: stage 1 and stage 2 do not need them)
+        if ((dim_max >= 1 && c->key_bits + lb > 64) || bits_for((u64)n) + tb > 64)
             r = RIPS_EOVERFLOW;
     }
     if (r != RIPS_OK) { rips_free(c); return r; }

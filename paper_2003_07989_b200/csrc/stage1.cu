@@ -587,17 +587,38 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
                         const int xs = __shfl_sync(RIPS_FULL_MASK, xo, src);
                         const int v1s = __shfl_sync(RIPS_FULL_MASK, r1o, src);
                         const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
+                        // (four groups of 32 vertices per round: the loads of a round are independent, so a column
+                        // without any cofacet of equal diameter -- a scan of all n vertices -- waits for HBM n/128
+                        // times, not n/32 times; that scan is what binds the kernel when n is in the thousands)
                         int res = -1;
-                        for (int base = n - 1 - kend; base >= 0; base -= 32) {
+                        int base = n - 1 - kend;
+                        if (base >= 0) { // the next 32 vertices first: most open lanes end here
                             const int vv = base - lane;
-                            bool ok = false;
+                            u32 m0 = 0u;
                             if (vv >= 0) {
-                                u32 m = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
-                                if (M > 2) m = min(m, (u32)u2[vv]);
-                                ok = m >= ks;
+                                m0 = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                                if (M > 2) m0 = min(m0, (u32)u2[vv]);
                             }
-                            const u32 bb = __ballot_sync(RIPS_FULL_MASK, ok);
-                            if (bb) { res = base - (__ffs(bb) - 1); break; }
+                            const u32 bb = __ballot_sync(RIPS_FULL_MASK, m0 >= ks); // (ks >= 1: an absent vertex never passes)
+                            if (bb) res = base - (__ffs(bb) - 1);
+                            base -= 32;
+                        }
+                        for (; base >= 0 && res < 0; base -= 128) {
+                            u32 mm[4];
+#pragma unroll
+                            for (int g = 0; g < 4; ++g) {
+                                const int vv = base - 32 * g - lane;
+                                mm[g] = 0u;
+                                if (vv >= 0) {
+                                    mm[g] = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                                    if (M > 2) mm[g] = min(mm[g], (u32)u2[vv]);
+                                }
+                            }
+#pragma unroll
+                            for (int g = 0; g < 4; ++g) {
+                                const u32 bb = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
+                                if (bb && res < 0) res = base - 32 * g - (__ffs(bb) - 1);
+                            }
                         }
                         if (lane == src) fv = res;
                     }
