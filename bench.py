@@ -50,6 +50,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k-1]; 2 is the one the metric is quoted on")
     ap.add_argument("--n", type=int, default=None, help="point count override (config 6, the second workload of PAPER.md:719-729: n = 1000 .. 20000)")
+    ap.add_argument("--mode", type=int, default=0, help="0 auto, 1 dense, 2 sparse (rips_set_mode)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
@@ -301,6 +302,7 @@ def run_b200(args):
 
     # ---- resident context; one full computation provides the clearing sets (and the barcode time)
     g = rips.Rips(dev, w.n, D, w.threshold)
+    g.set_mode(args.mode)
     t0 = time.perf_counter()
     compute_all(g, w, reduce_upto)
     torch.cuda.synchronize()
@@ -417,6 +419,7 @@ def run_b200(args):
         barrier()
         t0 = time.perf_counter()
         h = rips.Rips(host.numpy(), w.n, D, w.threshold, workspace=workspace)
+        h.set_mode(args.mode)
         compute_all(h, w, reduce_upto)
         bars = [h.barcodes(d) for d in range(0, reduce_upto + 1)]
         torch.cuda.synchronize()
@@ -507,6 +510,7 @@ def run_b200(args):
                                                             "n_nonapparent", "n_slots", "sort_passes",
                                                             "pair_sort_passes", "key_bits", "index_bits")} for d in range(1, D + 1)},
                 "device_bytes": g.device_bytes(), "parallelism": "replicas" if world > 1 else "single"}
+        line["mode"] = {0: "auto", 1: "dense", 2: "sparse"}[args.mode] + (" (sparse path taken)" if stats[D]["n_slots"] != comb(w.n, D + 1) and stats[D]["n_removed_by_diameter"] > 0 and stats[D]["n_slots"] == stats[D]["n_columns"] + stats[D]["n_cleared"] else "")
         if args.config == 6:
             import math
             closed = 1 - (math.sqrt(math.pi) / 2) * math.exp(math.lgamma(w.n - 1) - math.lgamma(w.n - 0.5))

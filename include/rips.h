@@ -134,6 +134,16 @@ int64_t rips_last_required_bytes(void);
 int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, float threshold, void* workspace_dev,
               int64_t workspace_bytes, void* stream);
 
+/* Which stage 1 the context runs; to be called before the first rips_stage1 / rips_compute.
+ *   RIPS_MODE_DENSE   every one of the C(n, d+1) combinatorial indices is enumerated (Algorithms 7-8 as printed);
+ *   RIPS_MODE_SPARSE  the sparse option of the paper (PAPER.md:395-437 Algorithm 5, :591, :932-934): neighbour lists of
+ *                     the edges within the threshold, the simplices of dimension d made from those of dimension d-1,
+ *                     cofacets from common neighbours; memory and time follow the size of the complex, not C(n, d+1);
+ *   RIPS_MODE_AUTO    (default) sparse iff the threshold admits less than 5 % of the edges (and n >= 64).
+ * Every array either mode exposes is the same (the tests compare both with the oracle). */
+enum { RIPS_MODE_AUTO = 0, RIPS_MODE_DENSE = 1, RIPS_MODE_SPARSE = 2 };
+int rips_set_mode(rips_ctx* ctx, int mode);
+
 /* Dimension 0 .. dim_max, all stages: dim 0, then per d: stage 1, stage 2, reduction. */
 int rips_compute(rips_ctx* ctx);
 

@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librips_b200.so")
-SOURCES = ["rips.cu", "radix_sort.cu", "stage1.cu", "stage2.cu", "dim0.cu", "init.cu", "reduce.cu"]
+SOURCES = ["rips.cu", "radix_sort.cu", "stage1.cu", "stage2.cu", "dim0.cu", "init.cu", "reduce.cu", "sparse.cu"]
 HEADERS = ["common.cuh", "kernels.cuh", "apparent.cuh", "radix_sort.cuh", os.path.join("..", "..", "include", "rips.h")]
 
 

@@ -7,7 +7,7 @@
 
 namespace {
 
-__global__ void prep_edges_kernel(float* __restrict__ dist, i64 E, u64* __restrict__ rec, int* bad)
+__global__ void prep_edges_kernel(float* __restrict__ dist, i64 E, u64* __restrict__ rec, int* bad, float threshold, u64* n_over)
 {
     i64 e = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= E) return;
@@ -15,6 +15,13 @@ __global__ void prep_edges_kernel(float* __restrict__ dist, i64 E, u64* __restri
     if (x == 0.0f) x = 0.0f; // -0 -> +0 (the comparison is true for both zeros)
     if (!(x >= 0.0f) || isinf(x)) { atomicOr(bad, 1); x = 0.0f; }
     dist[e] = x;
+    // every value above the threshold is ranked as ONE class (key 0, "value" +inf): no simplex that holds such an edge
+    // is ever kept, so their order among themselves is never looked at, and the keys of a thresholded input need only
+    // as many bits as it has admissible values (fewer sort passes; records that fit 64 bits for larger n)
+    if (x > threshold) {
+        x = __int_as_float(0x7f800000);
+        atomicAdd((unsigned long long*)n_over, 1ull); // (the compiler aggregates this per warp)
+    }
     // non-negative floats order like their bit patterns; invert so that ascending = value descending
     rec[e] = ((u64)(~__float_as_uint(x)) << 32) | (u64)e;
 }
@@ -107,10 +114,10 @@ cudaError_t launch_build_full_keys(const u32* K, int n, int pitch, void* Kf, int
     return cudaGetLastError();
 }
 
-cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, cudaStream_t st)
+cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, float threshold, u64* n_over, cudaStream_t st)
 {
     if (E == 0) return cudaSuccess;
-    prep_edges_kernel<<<(unsigned)((E + 255) / 256), 256, 0, st>>>(dist, E, rec, bad);
+    prep_edges_kernel<<<(unsigned)((E + 255) / 256), 256, 0, st>>>(dist, E, rec, bad, threshold, n_over);
     return cudaGetLastError();
 }
 

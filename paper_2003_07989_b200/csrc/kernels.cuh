@@ -23,7 +23,9 @@
 
 // ------------------------------------------------------------------ init.cu
 // rec[e] = (~bits(dist[e]) << 32) | e ; dist canonicalised in place (-0 -> +0); *bad |= 1 on NaN / inf / negative
-cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, cudaStream_t st);
+// (values above the threshold are all ranked as one class, +inf)
+// *n_over += number of such edges
+cudaError_t launch_prep_edges(float* dist, i64 E, u64* rec, int* bad, float threshold, u64* n_over, cudaStream_t st);
 // sorted rec (value descending, e ascending) -> K[e] = dense rank, values[rank]; *n_distinct
 cudaError_t launch_rank_edges(const u64* rec_sorted, i64 E, u32* K, float* values, u64* status, u32* ticket,
                               u64* n_distinct, cudaStream_t st);
@@ -87,13 +89,52 @@ struct Stage1Params {
     FusedHist fh_cols;   // digit histogram of the filtration sort (over every slot written to cols_out)
     FusedHist fh_pairs;  // digit histogram of the partition of pairs_out by v
 };
-int stage1_chunk(u64 total, int compact, double est_survival, int retry);
+int stage1_chunk(u64 total, int compact, double est_survival, int retry, int sms);
 int stage1_stage_cap();
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
 // bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask, i < min(n_rows, *n_dev) (n_dev may be NULL);
 // records with (rows[i] >> sent_shift) == sent are skipped (sent_shift < 0: none)
 cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, const u64* n_dev, int shift, u64 mask, int sent_shift,
                                 u64 sent, cudaStream_t st);
+
+// ------------------------------------------------------------------ sparse.cu (the sparse path, Algorithm 5)
+struct SparseExpand {
+    const u64* in;    // simplices of MP vertices as vertex words (NULL for MP = 1: the vertices 0..n_in-1)
+    i64 n_in;
+    const void* Kf;
+    int pitch, vbits;
+    u32 thr1;         // an edge is admissible iff its entry of Kf is >= thr1
+    const u64* off;   // CSR of the admissible edges: off[n+1], adj ascending per vertex
+    const u32* adj;
+    u32* cnt;         // [n_in] simplices made from each input simplex (count pass)
+    const u64* pos;   // [n_in] exclusive scan of cnt (write pass)
+    u64* out;         // simplices of MP+1 vertices, grouped by input simplex, the new (top) vertex ascending
+};
+struct SparseParams {
+    const u64* simp;  // all simplices of M vertices within the threshold, vertex words, increasing combinatorial index
+    i64 n_simp;
+    const void* Kf;
+    int pitch, n;
+    BinomTable bt;
+    int vbits, lowbits, tbits;
+    u32 sentinel_key;
+    const u64* off;
+    const u32* adj;
+    const u64* c_reg; i64 n_reg; u64 reg_mask;   // clearing set: the three sorted layers of dimension d-1's pivots
+    const u64* c_irr; i64 n_irr;
+    const u64* c_red; i64 n_red;
+    u64* cols_out;    // [n_simp] column record or sentinel (slot = position in simp)
+    u64* pairs_out;   // [n_simp] regular pair record or sentinel
+    u64* irr_out; u64* non_out; u64 irr_cap, non_cap;
+    u64* counters;    // S1C_*
+};
+i64 sparse_scan_tiles(i64 n);
+cudaError_t launch_csr_count(const void* Kf, int kf_u16, int n, int pitch, u32 thr1, u32* deg, cudaStream_t st);
+cudaError_t launch_csr_scan(const u32* deg, int n, u64* off, cudaStream_t st);
+cudaError_t launch_csr_fill(const void* Kf, int kf_u16, int n, int pitch, u32 thr1, const u64* off, u32* adj, cudaStream_t st);
+cudaError_t launch_scan_counts(const u32* cnt, i64 n, u64* pos, u64* status, u32* ticket, cudaStream_t st);
+cudaError_t launch_expand(int MP, int kf_u16, const SparseExpand& e, bool write, cudaStream_t st);
+cudaError_t launch_sparse_apparent(int M, int kf_u16, const SparseParams& p, cudaStream_t st);
 
 // ------------------------------------------------------------------ pair store, unpack, lookup (stage2.cu)
 // The two sorted layers of apparent pairs of one dimension (the third layer, the pivots found by the

@@ -150,6 +150,10 @@ struct DimState {
     bool caps_valid = false;      // a run of this dimension has fitted its lists: the sizes are known to suffice
     u64 irr_cap = 0, non_cap = 0; // capacities of the two small lists (records)
     int chunk_retry = 0, attempts = 0;
+    DevBuf simpA, simpB;          // sparse path: all simplices of this dimension within the threshold (vertex words)
+    const u64* simp = nullptr;    // ... in increasing combinatorial index
+    i64 n_simp = -1;
+    i64 sparse_over = 0;          // sparse path: candidates never enumerated (diameter above the threshold)
     // stage 1 + stage 2 of this dimension as one CUDA graph (captured once the sizes are known to fit)
     cudaGraphExec_t graph = nullptr;
     u64 graph_sig = 0;
@@ -211,6 +215,11 @@ struct rips_ctx {
     u64* h_counters = nullptr; // pinned
     u64* h_dimcnt = nullptr;   // pinned: 8 u64 per dimension (DimState::h_cnt)
     u32 n_distinct = 0, thr_key = 0;
+    double edge_share = 1.0; // share of the edges the threshold admits
+    int mode = 0;            // RIPS_MODE_*
+    bool sparse = false, mode_locked = false; // the path stage 1 takes, fixed by the first stage 1
+    DevBuf sp_deg, sp_off, sp_adj, sp_cnt, sp_pos, sp_status; // sparse path: CSR of the admissible edges, expansion scratch
+    bool have_csr = false;
     int key_bits = 1;
     DevBuf sort_scratch, sort_scratch2, sort_scratch3;
     // dim 0
@@ -428,17 +437,163 @@ int finish_counts(rips_ctx* c, int d)
         return finish_counts(c, d);
     }
     s.attempts = 0;
-    s.caps_valid = true;
+    s.caps_valid = !c->sparse; // (the sparse path sizes its arrays by what it finds, run by run: it stays synchronous)
     s.len = s.compact ? (i64)h[S1C_KEPT] : (i64)(s.total - h[S1C_OVER] - h[S1C_CLEARED]); // slot mode counts what it drops
     s.n_reg = (i64)h[S1C_REGULAR];
     s.n_irr = (i64)ni;
     s.n_non = (i64)nn;
     s.stats.n_columns = s.len;
-    s.stats.n_removed_by_diameter = (i64)h[S1C_OVER];
+    s.stats.n_removed_by_diameter = (i64)h[S1C_OVER] + s.sparse_over;
     s.stats.n_cleared = (i64)h[S1C_CLEARED];
     s.stats.n_apparent = s.n_reg + s.n_irr;
     s.stats.n_nonapparent = s.n_non;
     s.stats.n_regular = s.n_reg;
+    return RIPS_OK;
+}
+
+// ------------------------------------------------------------------------------------------ stage 1, sparse path
+int ensure_csr(rips_ctx* c)
+{
+    if (c->have_csr) return RIPS_OK;
+    const int n = (int)c->n;
+    const u32 thr1 = c->thr_key + 1u;
+    RC(ensure(c, c->sp_deg, (size_t)n * 4));
+    RC(ensure(c, c->sp_off, (size_t)(n + 1) * 8));
+    CU(launch_csr_count(c->d_Kf, c->kf_u16, n, c->kf_pitch, thr1, (u32*)c->sp_deg.p, c->stream));
+    CU(launch_csr_scan((const u32*)c->sp_deg.p, n, (u64*)c->sp_off.p, c->stream));
+    CU(cudaMemcpyAsync(c->h_counters, (u64*)c->sp_off.p + n, 8, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    const u64 total = c->h_counters[0];
+    RC(ensure(c, c->sp_adj, (size_t)total * 4));
+    CU(launch_csr_fill(c->d_Kf, c->kf_u16, n, c->kf_pitch, thr1, (const u64*)c->sp_off.p, (u32*)c->sp_adj.p, c->stream));
+    c->launches += 3;
+    c->have_csr = true;
+    return RIPS_OK;
+}
+
+// Sparse stage 1 (sparse.cu): the simplices of dimension d from those of dimension d-1 and the neighbour lists, in
+// increasing combinatorial index; then one thread per simplex (key, clearing, apparent test) writes the records the
+// dense kernels write in slot mode, the position in the list being the slot.  The sorts that follow are the dense ones.
+int run_stage1_sparse(rips_ctx* c, int d)
+{
+    DimState& s = c->dims[d];
+    DimState& prev = c->dims[d - 1];
+    const i64 n = c->n;
+    const int pvbits = bits_for((u64)n);
+    RC(ensure_csr(c));
+    // ---- the simplex list L_d
+    const int MP = d; // vertices of the simplices it is made from
+    const u64* in = nullptr;
+    i64 n_in = n;
+    if (d >= 2) {
+        if (prev.n_simp < 0 || (prev.n_simp > 0 && !prev.simp)) {
+            g_last_error = "rips_stage1: the sparse path needs the previous dimension's simplex list (run its stage 1 in sparse mode)";
+            return RIPS_EINVAL;
+        }
+        in = prev.simp;
+        n_in = prev.n_simp;
+    }
+    i64 total = 0;
+    if (n_in > 0) {
+        RC(ensure(c, c->sp_cnt, (size_t)n_in * 4));
+        RC(ensure(c, c->sp_pos, (size_t)(n_in + 1) * 8));
+        RC(ensure(c, c->sp_status, (size_t)sparse_scan_tiles(n_in) * 8 + 64));
+        SparseExpand e;
+        e.in = in; e.n_in = n_in; e.Kf = c->d_Kf; e.pitch = c->kf_pitch; e.vbits = c->vbits; e.thr1 = c->thr_key + 1u;
+        e.off = (const u64*)c->sp_off.p; e.adj = (const u32*)c->sp_adj.p; e.cnt = (u32*)c->sp_cnt.p; e.pos = (const u64*)c->sp_pos.p; e.out = nullptr;
+        CU(launch_expand(MP, c->kf_u16, e, false, c->stream));
+        CU(cudaMemsetAsync(c->sp_status.p, 0, (size_t)sparse_scan_tiles(n_in) * 8 + 64, c->stream));
+        u64* status = (u64*)c->sp_status.p + 8;
+        CU(launch_scan_counts((const u32*)c->sp_cnt.p, n_in, (u64*)c->sp_pos.p, status, (u32*)c->sp_status.p, c->stream));
+        CU(cudaMemcpyAsync(c->h_counters, (u64*)c->sp_pos.p + n_in, 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        total = (i64)c->h_counters[0];
+        c->launches += 2;
+        if (total > 0) {
+            RC(ensure(c, s.simpA, (size_t)total * 8));
+            RC(ensure(c, s.simpB, (size_t)total * 8));
+            e.out = (u64*)s.simpA.p;
+            CU(launch_expand(MP, c->kf_u16, e, true, c->stream));
+            c->launches += 1;
+            // stable partition by the new (top) vertex: increasing combinatorial index
+            SortPlan pp = sort_make_plan(MP * c->vbits, (MP + 1) * c->vbits);
+            RC(ensure(c, c->sort_scratch, sort_scratch_bytes(total, pp)));
+            u64* res = nullptr;
+            CU(sort_u64((u64*)s.simpA.p, (u64*)s.simpB.p, total, pp, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+            s.simp = res;
+        }
+    }
+    s.n_simp = total;
+    s.sparse_over = (i64)s.total - total;
+    s.compact = 1;
+    s.slots = total;
+    s.stats.n_slots = total;
+    ev_record(c, s, EV_S1_BITMAP);
+    if (total == 0) {
+        ev_record(c, s, EV_S1_ENUM); ev_record(c, s, EV_S1_SORTBEG); ev_record(c, s, EV_S1_HIST); ev_record(c, s, EV_S1_SORT); ev_record(c, s, EV_S1_END);
+        s.len = 0; s.n_reg = s.n_irr = s.n_non = 0;
+        s.stats.n_removed_by_diameter = (i64)s.total;
+        s.irr_cap = s.non_cap = 0;
+        s.pair_plan = sort_make_plan(s.tbits, s.tbits + pvbits);
+        s.pair_fused = false;
+        s.have_s1 = true;
+        s.pairs_fresh = true;
+        return RIPS_OK;
+    }
+    RC(ensure(c, s.d_cnt, 128));
+    u64* const d_cnt = (u64*)s.d_cnt.p;
+    RC(ensure(c, s.colsA, (size_t)total * 8));
+    RC(ensure(c, s.colsB, (size_t)total * 8));
+    RC(ensure(c, s.pairsA, (size_t)total * 8));
+    s.irr_cap = std::max<u64>(s.irr_cap, std::max<u64>(4096, (u64)total / 8));
+    s.non_cap = std::max<u64>(s.non_cap, std::max<u64>(4096, (u64)total / 8));
+    RC(ensure(c, s.irrA, (size_t)s.irr_cap * 8));
+    RC(ensure(c, s.nonA, (size_t)s.non_cap * 8));
+    SparseParams p;
+    p.simp = s.simp; p.n_simp = total; p.Kf = c->d_Kf; p.pitch = c->kf_pitch; p.n = (int)n; p.bt = c->bt();
+    p.vbits = c->vbits; p.lowbits = s.lowbits; p.tbits = s.tbits; p.sentinel_key = c->n_distinct;
+    p.off = (const u64*)c->sp_off.p; p.adj = (const u32*)c->sp_adj.p;
+    p.c_reg = (d >= 2) ? prev.reg : nullptr; p.n_reg = (d >= 2) ? prev.n_reg : 0;
+    p.reg_mask = (prev.tbits >= 64) ? ~0ull : ((1ull << prev.tbits) - 1ull);
+    p.c_irr = (d >= 2) ? prev.irr : nullptr; p.n_irr = (d >= 2) ? prev.n_irr : 0;
+    p.c_red = (const u64*)prev.red_t.p; p.n_red = prev.n_red;
+    p.cols_out = (u64*)s.colsA.p; p.pairs_out = (u64*)s.pairsA.p;
+    p.irr_out = (u64*)s.irrA.p; p.non_out = (u64*)s.nonA.p; p.irr_cap = s.irr_cap; p.non_cap = s.non_cap;
+    p.counters = d_cnt;
+    CU(cudaMemsetAsync(d_cnt, 0, 128, c->stream));
+    CU(launch_sparse_apparent(s.M, c->kf_u16, p, c->stream));
+    c->launches += 1;
+    ev_record(c, s, EV_S1_ENUM);
+    {
+        cudaStream_t sc = c->stream2 ? c->stream2 : c->stream;
+        if (sc != c->stream) {
+            CU(cudaEventRecord(c->ev_fused, c->stream));
+            CU(cudaStreamWaitEvent(sc, c->ev_fused, 0));
+        }
+        CU(cudaMemcpyAsync(s.h_cnt, d_cnt, 64, cudaMemcpyDeviceToHost, sc));
+        CU(cudaEventRecord(s.ev_cnt, sc));
+        s.counts_pending = true;
+        s.cnt_copied = true;
+    }
+    SortPlan plan = sort_make_plan(s.lowbits, s.lowbits + c->key_bits);
+    s.pair_plan = sort_make_plan(s.tbits, s.tbits + pvbits);
+    s.pair_fused = false;
+    RC(ensure(c, c->sort_scratch, sort_scratch_bytes(total, plan)));
+    RC(ensure(c, s.pair_scratch, sort_scratch_bytes(total, s.pair_plan)));
+    {
+        SortTimes st;
+        st.enabled = true;
+        st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
+        s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
+        u64* res = nullptr;
+        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, total, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, false));
+        s.cols = res;
+        ev_record(c, s, EV_S1_END);
+    }
+    s.stats.sort_passes = total > 1 ? plan.npasses : 0;
+    s.have_s1 = true;
+    s.pairs_fresh = true;
+    RC(finish_counts(c, d)); // the sparse path is synchronous: the sizes of the next steps come from these counts
     return RIPS_OK;
 }
 
@@ -496,6 +651,11 @@ int run_stage1(rips_ctx* c, int d)
         return RIPS_OK;
     }
     if (s.cnt_copied && c->stream2 && !c->capturing) CU(cudaStreamWaitEvent(c->stream, s.ev_cnt, 0)); // the previous run's copy of the counters
+    if (!c->mode_locked) {
+        c->sparse = c->mode == RIPS_MODE_SPARSE || (c->mode == RIPS_MODE_AUTO && c->thr_key != 0 && c->edge_share < 0.05 && c->n >= 64);
+        c->mode_locked = true;
+    }
+    if (c->sparse) return run_stage1_sparse(c, d);
     RC(ensure(c, s.d_cnt, 128)); // 8 u64 counters, then the kernel's tickets
     u64* const d_cnt = (u64*)s.d_cnt.p;
     u32* const d_tick = (u32*)(d_cnt + 8);
@@ -532,10 +692,10 @@ int run_stage1(rips_ctx* c, int d)
     // mode: without a threshold at least (n-d-1)/n of the candidates survive (only clearing drops
     // any), so every candidate keeps its slot; with one, estimate the surviving share from the share
     // q of admissible edges (q^(edges of the simplex)) and compact when most are dropped
-    const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
+    const double q = c->edge_share;
     const double est_survival = std::pow(q, (double)(s.M * (s.M - 1) / 2));
     s.compact = (c->thr_key != 0 && est_survival < 0.5) ? 1 : 0;
-    int chunk = stage1_chunk(s.total, s.compact, est_survival, s.chunk_retry);
+    int chunk = stage1_chunk(s.total, s.compact, est_survival, s.chunk_retry, c->sms);
     i64 tiles = (i64)((s.total + (u64)chunk - 1) / (u64)chunk);
     Stage1Params p;
     p.Kf = c->d_Kf;
@@ -887,7 +1047,7 @@ int check_dim(rips_ctx* c, int d, int lo)
 void free_dim(rips_ctx* c, DimState& s)
 {
     DevBuf* all[] = {&s.colsA, &s.colsB, &s.s1_status, &s.bitmap, &s.pairsA, &s.pairsB, &s.irrA, &s.irrB, &s.nonA, &s.nonB,
-                     &s.pair_scratch, &s.d_cnt, &s.rd_piv, &s.rd_colref, &s.rd_todo, &s.rd_htk, &s.rd_htv, &s.rd_arena, &s.rd_cnt,
+                     &s.pair_scratch, &s.d_cnt, &s.simpA, &s.simpB, &s.rd_piv, &s.rd_colref, &s.rd_todo, &s.rd_htk, &s.rd_htv, &s.rd_arena, &s.rd_cnt,
                      &s.rd_rec, &s.rd_rec2, &s.rd_bars, &s.red_t,
                      &s.red_s, &s.v_fdiam, &s.v_fcidx, &s.v_at, &s.v_as, &s.v_ndiam, &s.v_ncidx, &s.v_pt, &s.v_ps};
     for (DevBuf* b : all) release(c, *b);
@@ -922,7 +1082,7 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         RC(ensure(c, c->b_init_tmp, (size_t)E * 8));
         CU(cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
         CU(cudaMemsetAsync(c->d_tickets, 0, 32, c->stream));
-        CU(launch_prep_edges(c->d_dist, E, c->d_edges, (int*)(c->d_counters + 1), c->stream));
+        CU(launch_prep_edges(c->d_dist, E, c->d_edges, (int*)(c->d_counters + 1), c->threshold, c->d_counters + 2, c->stream));
         SortPlan plan = sort_make_plan(32, 64);
         RC(ensure(c, c->sort_scratch, sort_scratch_bytes(E, plan)));
         u64* res = nullptr;
@@ -932,8 +1092,9 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         CU(cudaMemsetAsync(c->b_init_status.p, 0, (size_t)rank_edges_tiles(E) * 8, c->stream));
         CU(launch_rank_edges(c->d_edges, E, c->d_K, c->d_values, (u64*)c->b_init_status.p, c->d_tickets, c->d_counters, c->stream));
         c->launches += 2;
-        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
+        c->edge_share = E ? (double)(E - (i64)c->h_counters[2]) / (double)E : 1.0;
         release(c, c->b_init_tmp);
         release(c, c->b_init_status);
         if ((int)c->h_counters[1] != 0) {
@@ -1098,7 +1259,7 @@ int rips_init(rips_ctx** out, const float* dist_lower, int64_t n, int dim_max, f
     }
     r = init_device_tables(c, dist_lower);
     if (r == RIPS_OK && !workspace_dev) {
-        const double q = c->n_distinct ? (double)(c->n_distinct - c->thr_key) / (double)c->n_distinct : 1.0;
+        const double q = c->edge_share;
         long double rest = 0;
         for (int d = 1; d <= dim_max; ++d) {
             const double surv = std::pow(q, (double)((d + 1) * d / 2));
@@ -1154,6 +1315,14 @@ void rips_free(rips_ctx* c)
 }
 
 int rips_dim0(rips_ctx* c) { return c ? run_dim0(c) : RIPS_EINVAL; }
+
+int rips_set_mode(rips_ctx* c, int mode)
+{
+    if (!c || mode < RIPS_MODE_AUTO || mode > RIPS_MODE_SPARSE) return RIPS_EINVAL;
+    if (c->mode_locked) { g_last_error = "rips_set_mode: a stage 1 has already run on this context"; return RIPS_EINVAL; }
+    c->mode = mode;
+    return RIPS_OK;
+}
 // Stage 1 + stage 2 of a dimension whose sizes are known to fit are one CUDA graph: ~45 kernels, memsets and copies on
 // three streams whose launch parameters no longer change (the counts they depend on are read on the device).  The
 // graph is captured by the first rips_stage1 call that finds the dimension in that state and replayed by the later

@@ -789,9 +789,9 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 // (est_survival x chunk) fill half the staging; a chunk that overflows is reported and the launch repeated
 // with chunk = S1_STAGE_CAP (retry != 0).
 int stage1_stage_cap() { return 256; }
-int stage1_chunk(u64 total, int compact, double est_survival, int retry)
+int stage1_chunk(u64 total, int compact, double est_survival, int retry, int sms)
 {
-    u64 c = (total / (148ull * 64) + 31) / 32 * 32;
+    u64 c = (total / ((u64)(sms > 0 ? sms : 148) * 64) + 31) / 32 * 32;
     if (c < 32) c = 32;
     if (!compact) return (int)(c > (u64)S1_CHUNK ? (u64)S1_CHUNK : c);
     const u64 cap = (u64)stage1_stage_cap();

@@ -144,6 +144,16 @@ def config(k: int, n: int | None = None) -> Workload:
                         "standard Gaussian in R^8, seed 4, threshold = enclosing radius")
     if k == 6:
         return second_workload(n or 5000)
+    if k == 7:
+        # the regime of the paper's sparse option (o3 with a threshold that keeps 0.00038 % of the
+        # possible simplices, Table 5): a point cloud under a threshold far below the enclosing radius.
+        # C(1700, 4) = 3.5e11 candidate tetrahedra (a 43 GB clearing bitmap, seconds of enumeration for the dense path,
+        # hours for the oracle's Algorithm 7); the complex itself has ~3.4e4 edges.  1700 is about the largest n whose
+        # reduction entries of dimension 3 (key + row index) still fit 64 bits.
+        n = n or 1700
+        return Workload(f"cfg7_sparse_cube3_n{n}", n, 3, float(np.float32(0.1777 * (1700.0 / n) ** (1.0 / 3.0))),
+                        euclidean_lower(cube_points(n, 3, 5)),
+                        "uniform in unit cube R^3, seed 5, threshold for a mean degree of ~40: sparse path only")
     raise ValueError(f"no config {k}")
 
 

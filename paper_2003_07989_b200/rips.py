@@ -19,7 +19,7 @@ RIPS_OK, RIPS_EINVAL, RIPS_EOVERFLOW, RIPS_ENOMEM, RIPS_ECUDA = 0, -1, -2, -3, -
 
 # every symbol include/rips.h declares (checked by tests/test_abi.py against the header)
 SYMBOLS = [
-    "rips_workspace_bytes", "rips_init", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce", "rips_import_pivots",
+    "rips_workspace_bytes", "rips_init", "rips_set_mode", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce", "rips_import_pivots",
     "rips_barcodes", "rips_filtration", "rips_apparent_pairs", "rips_nonapparent", "rips_pivots",
     "rips_pivot_lookup", "rips_stats", "rips_timings", "rips_device_bytes", "rips_workspace_in_use", "rips_kernel_launches",
     "rips_sort_u64", "rips_strerror", "rips_last_error", "rips_last_required_bytes", "rips_free",
@@ -70,7 +70,7 @@ def lib():
         l.rips_init.argtypes = [pp, vp, i64, i32, C.c_float, vp, i64, vp]
         for f in ("rips_compute", "rips_dim0"):
             getattr(l, f).argtypes = [vp]
-        for f in ("rips_stage1", "rips_stage2", "rips_reduce"):
+        for f in ("rips_stage1", "rips_stage2", "rips_reduce", "rips_set_mode"):
             getattr(l, f).argtypes = [vp, i32]
         for f in ("rips_barcodes",):
             getattr(l, f).argtypes = [vp, i32, pp, pi64]
@@ -188,6 +188,11 @@ class Rips:
         self.free()
 
     # -- compute
+    def set_mode(self, mode):
+        """0 = auto, 1 = dense, 2 = sparse (RIPS_MODE_*); before the first stage 1."""
+        _check(lib().rips_set_mode(self._h, {"auto": 0, "dense": 1, "sparse": 2}.get(mode, mode)), "rips_set_mode")
+        return self
+
     def compute(self):
         _check(lib().rips_compute(self._h), "rips_compute")
         return self

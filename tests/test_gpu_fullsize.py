@@ -141,6 +141,75 @@ def _compare_dimension(g, o, d, tag):
     assert st["n_essential"] == o[d]["essential"].size and st["n_reduced_pivots"] == o[d]["red_t"].size, tag
 
 
+def test_config4_through_both_paths(R):
+    """Config 4 (1000 points, threshold 0.15: 1.2 % of the edges) at full size through the sparse path (what
+    RIPS_MODE_AUTO picks for it) and through the dense path: every array of every dimension against the oracle."""
+    w = inputs.config(4)
+    o = oracle.barcodes(w.dist, w.n, w.dim_max, w.threshold)
+    for mode in ("sparse", "dense"):
+        with R.Rips(w.dist, w.n, w.dim_max, w.threshold) as g:
+            g.set_mode(mode)
+            g.compute()
+            for d in range(0, w.dim_max + 1):
+                _compare_dimension(g, o, d, f"{w.name} {mode} d={d}")
+            st = g.stats(2)
+            assert st["n_candidates"] == comb(w.n, 3) and st["n_slots"] == (o[2]["counts"]["kept"] + o[2]["counts"]["cleared"] if mode == "sparse" else st["n_columns"])
+
+
+def test_config7_sparse_only(R):
+    """1700 points under a threshold that admits ~2.4 % of the edges, dimensions 1..3: C(1700,4) = 3.5e11 candidate
+    tetrahedra, which the oracle's Algorithm 7 cannot enumerate in a test's time (the dense path needs seconds and a
+    43 GB bitmap).  Dimension 1 against the
+    oracle; above it what can be checked independently: the number of simplices the sparse path lists against clique
+    counts of the threshold graph (numpy), the orders of the arrays, zero persistence of sampled apparent pairs, and
+    the sparse path of a 500-point version of the same cloud against the oracle in full (same code path, sizes the
+    oracle reaches)."""
+    import torch
+    w = inputs.config(7)
+    n = w.n
+    sq = inputs.square_from_lower(w.dist, n)
+    A = ((sq <= np.float32(w.threshold)) & ~np.eye(n, dtype=bool))
+    Af = A.astype(np.float32)
+    n_edges = int(A.sum()) // 2
+    n_tri = int(round(float(np.trace(Af @ Af @ Af)) / 6.0))
+    iu, ju = np.nonzero(np.triu(A, 1))
+    n_tet = 0
+    for a, b in zip(iu, ju):                      # 4-cliques: edges inside the common neighbourhood of every edge, / 6
+        cn = np.nonzero(A[a] & A[b])[0]
+        if cn.size >= 2:
+            n_tet += int(A[np.ix_(cn, cn)].sum()) // 2
+    n_tet //= 6
+    o1 = oracle.barcodes(w.dist, n, 1, w.threshold)
+    with R.Rips(w.dist, n, 3, w.threshold) as g:
+        g.compute()                               # RIPS_MODE_AUTO: sparse
+        _compare_dimension(g, o1, 0, "cfg7 d=0")
+        _compare_dimension(g, o1, 1, "cfg7 d=1")
+        for d, cliques in ((1, n_edges), (2, n_tri), (3, n_tet)):
+            st = g.stats(d)
+            assert st["n_slots"] == cliques == st["n_columns"] + st["n_cleared"], (d, st, cliques)
+            assert st["n_candidates"] == comb(n, d + 1) and st["n_removed_by_diameter"] == comb(n, d + 1) - cliques
+            assert st["n_apparent"] + st["n_nonapparent"] == st["n_columns"]
+            assert st["n_cleared"] == g.pivots(d - 1)[0].numel()   # every pivot row of dimension d-1 is a simplex of the complex
+            fd, fc = g.filtration(d)
+            dd = fd[1:] - fd[:-1]
+            assert bool((dd <= 0).all()) and bool((fc[1:][dd == 0] > fc[:-1][dd == 0]).all())
+            assert float(fd.max()) <= w.threshold
+            at, as_ = g.apparent_pairs(d)
+            assert bool((at[1:] > at[:-1]).all())
+            idx = torch.linspace(0, at.numel() - 1, 60).long()
+            for t, s_ in zip(at[idx].tolist(), as_[idx].tolist()):
+                assert oracle.diameter(w.dist, t, d + 2, n) == oracle.diameter(w.dist, s_, d + 1, n)
+            pt, ps = g.pivots(d)
+            assert pt.numel() + st["n_essential"] == st["n_columns"] and torch.unique(ps).numel() == ps.numel()
+    ws = inputs.config(7, 500)
+    o = oracle.barcodes(ws.dist, ws.n, 3, ws.threshold)
+    with R.Rips(ws.dist, ws.n, 3, ws.threshold) as g:
+        g.set_mode("sparse")
+        g.compute()
+        for d in range(0, 4):
+            _compare_dimension(g, o, d, f"{ws.name} d={d}")
+
+
 @pytest.mark.parametrize("k", [2, 4, 5])
 def test_full_size_barcodes(R, k):
     """BASELINE.json configs 2, 4, 5 at full size through rips_compute: EVERY array of EVERY dimension -- filtration,

@@ -25,9 +25,11 @@ def _np(t):
     return t.cpu().numpy()
 
 
-def check_against_oracle(R, low, n, dim_max, thr=inf, what=""):
+def check_against_oracle(R, low, n, dim_max, thr=inf, what="", mode=None):
     o = oracle.barcodes(low, n, dim_max, thr)
     with R.Rips(low, n, dim_max, thr) as g:
+        if mode is not None:
+            g.set_mode(mode)
         g.compute()
         # dimension 0
         pt, ps = g.pivots(0)
@@ -75,6 +77,46 @@ def test_shadow_configs(R, k, n):
     if k == 4:
         thr = float(np.float32(np.quantile(w.dist, 0.25)))
     check_against_oracle(R, w.dist, n, w.dim_max, thr, w.name)
+
+
+@pytest.mark.parametrize("k,n,q", [(1, 40, 0.1), (2, 30, 0.3), (3, 50, 0.05), (4, 120, 0.04), (5, 48, 0.5), (1, 70, 1.0), (4, 300, 0.02)])
+def test_sparse_path_shadow_configs(R, k, n, q):
+    """The sparse path (RIPS_MODE_SPARSE: neighbour lists, simplices of dimension d from those of dimension d-1,
+    cofacets from common neighbours) on the five distributions under thresholds that admit a share q
+    of the edges (q = 1: the full complex through the sparse path): every array against the oracle, and the dense path
+    on the same input gives the same counts."""
+    w = inputs.config(k, n)
+    thr = inf if q == 1.0 else float(np.float32(np.quantile(w.dist, q)))
+    dm = w.dim_max if n <= 120 else 2
+    check_against_oracle(R, w.dist, n, dm, thr, f"sparse {w.name} q={q}", mode="sparse")
+    check_against_oracle(R, w.dist, n, dm, thr, f"dense {w.name} q={q}", mode="dense")
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_sparse_path_randomized(R, seed):
+    rng = np.random.default_rng(3000 + seed)
+    n = int(rng.integers(5, 90))
+    dim_max = int(rng.integers(1, 4)) if n <= 40 else int(rng.integers(1, 3))
+    regime = seed % 3
+    if regime == 0:
+        low = inputs.random_matrix_lower(n, 150 + seed)
+    elif regime == 1:
+        low = inputs.small_integer_lower(n, 160 + seed, hi=int(rng.integers(2, 9)))
+    else:
+        low = inputs.euclidean_lower(inputs.cube_points(n, int(rng.integers(1, 4)), 170 + seed))
+    q = float(rng.choice([1.0, 0.6, 0.3, 0.1, 0.03, 0.0]))
+    thr = inf if q == 1.0 else float(np.float32(np.quantile(low, q)))
+    check_against_oracle(R, low, n, dim_max, thr, f"sparse seed {seed}: n={n} dim_max={dim_max} regime={regime} q={q}", mode="sparse")
+
+
+def test_mode_is_fixed_by_the_first_stage1(R):
+    w = inputs.config(1, 20)
+    with R.Rips(w.dist, w.n, 1) as g:
+        g.dim0()
+        g.stage1(1)
+        with pytest.raises(R.RipsError) as e:
+            g.set_mode("sparse")
+        assert e.value.code == R.RIPS_EINVAL
 
 
 @pytest.mark.parametrize("name", ["constant", "cyclic", "cross", "descending", "smallint", "zeros"])
