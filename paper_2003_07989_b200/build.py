@@ -33,20 +33,45 @@ def needs_build() -> bool:
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
-        return LIB
-    tmp = LIB + f".{os.getpid()}.tmp"
+STRESS_LIB = os.path.join(HERE, "librips_b200_stress.so")
+STRESS_FLAGS = ["-DRIPS_STRESS", "-DRIPS_SORT_THREADS=256", "-DRIPS_SORT_IPT=2", "-DRIPS_SORT_MIN_BLOCKS=3", "-DRIPS_SORT_RANK_BATCH=2"]
+
+
+def _compile(out: str, extra, verbose: bool) -> None:
+    tmp = out + f".{os.getpid()}.tmp"
     cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC,-O3", "--use_fast_math" if False else "-Xcompiler", "-Wall",
-           "-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
+           "-shared", "-Xcompiler", "-fPIC,-O3", "-Xcompiler", "-Wall"] + list(extra) + \
+          ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
+    os.replace(tmp, out)
+
+
+def _stale(out: str) -> bool:
+    if not os.path.exists(out):
+        return True
+    t = os.path.getmtime(out)
+    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if force or needs_build():
+        _compile(LIB, [], verbose)
     return LIB
+
+
+def build_stress(force: bool = False) -> str:
+    """The same sources with -DRIPS_STRESS: sort tiles of 512 records, short chunks in compact mode, pseudo-random
+    delays in front of every publication of the chained scans and of the lock-free reduction.  Test infrastructure
+    (tests/test_gpu_parity.py::test_stress_build): same C ABI, same results, different schedules."""
+    if force or _stale(STRESS_LIB):
+        _compile(STRESS_LIB, STRESS_FLAGS, False)
+    return STRESS_LIB
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--stress" in sys.argv:
+        print(build_stress(force="--force" in sys.argv))

@@ -30,6 +30,19 @@ __device__ __forceinline__ void st_volatile_u64(u64* p, u64 v)
     asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// Stress build (-DRIPS_STRESS, paper_2003_07989_b200/build.py build_stress): tiny tiles and pseudo-random delays in
+// front of every publication of a chained scan and of the lock-free reduction, so that the orders in which tiles and
+// columns publish are shuffled far beyond what a normal run produces (compute-sanitizer is not available on the pool).
+#ifdef RIPS_STRESS
+__device__ __forceinline__ void stress_jitter(u32 salt)
+{
+    u32 h = (salt * 2654435761u + blockIdx.x * 2246822519u + (u32)clock64()) * 3266489917u;
+    __nanosleep((h >> 21) & 2047u);
+}
+#else
+__device__ __forceinline__ void stress_jitter(u32) {}
+#endif
+
 __device__ __forceinline__ u64 warp_sum_u64(u64 v)
 {
 #pragma unroll
@@ -52,6 +65,7 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, i64 tile, u64 agg
         if (lane == 0) st_volatile_u64(status, LB_FLAG_INC | aggregate);
         return 0;
     }
+    stress_jitter((u32)tile);
     if (lane == 0) st_volatile_u64(status + tile, LB_FLAG_AGG | aggregate);
     u64 excl = 0;
     i64 look = tile - 1;
@@ -71,6 +85,7 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, i64 tile, u64 agg
         excl += warp_sum_u64(s & LB_VALUE_MASK);
         look -= 32;
     }
+    stress_jitter((u32)tile + 77u);
     if (lane == 0) st_volatile_u64(status + tile, LB_FLAG_INC | (excl + aggregate));
     return excl;
 }

@@ -197,6 +197,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, c
                 run += c;
             }
             my_count = (tid == nbins - 1) ? run - (u32)n_pad : run;
+            stress_jitter((u32)tile * 31u + (u32)tid);
             st_volatile_u64(status + tile * nbins + tid, (tile == 0 ? LB_FLAG_INC : LB_FLAG_AGG) | (u64)my_count);
         }
         // block scan of `run` over the first MAX_BINS threads (8 warps)
@@ -264,6 +265,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, c
                     if (fin) break;
                 }
             }
+            stress_jitter((u32)tile * 17u + (u32)tid);
             st_volatile_u64(status + tile * nbins + tid, LB_FLAG_INC | (excl + (u64)my_count));
         }
         goff[tid] = __ldg(global_base + tid) + excl - (u64)bin_start[tid];

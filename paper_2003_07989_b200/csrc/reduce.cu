@@ -989,6 +989,7 @@ __global__ void __launch_bounds__(RD_THREADS) reduce_kernel(const ReduceParams p
                         p.colref[cur] = RD_REF(roff, (u64)rlen, 1);
                         p.piv[cur] = pe;
                         __threadfence();
+                        stress_jitter((u32)cur);
                         sh.bc_u64[1] = (u64)atomicCAS(p.ht_vals + slot, owner, (u32)cur);
                         // the working column is now that published copy, by reference
                         ws.ptr[0] = p.arena + roff; ws.pos[0] = 0; ws.len[0] = (u32)rlen; ws.own[0] = 0; ws.head[0] = pe; ws.wbase[0] = 0xffffffffu; ws.nruns = 1;

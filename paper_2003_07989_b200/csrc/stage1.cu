@@ -788,7 +788,11 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
 // chunks is a link of the look-back chain: the chunk is sized so that the expected survivors
 // (est_survival x chunk) fill half the staging; a chunk that overflows is reported and the launch repeated
 // with chunk = S1_STAGE_CAP (retry != 0).
+#ifdef RIPS_STRESS
+int stage1_stage_cap() { return 64; }   // short chunks: many links in compact mode's look-back chain
+#else
 int stage1_stage_cap() { return 256; }
+#endif
 int stage1_chunk(u64 total, int compact, double est_survival, int retry, int sms)
 {
     u64 c = (total / ((u64)(sms > 0 ? sms : 148) * 64) + 31) / 32 * 32;

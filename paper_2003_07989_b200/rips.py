@@ -96,6 +96,14 @@ def lib():
     return _lib
 
 
+def use_library(path=None):
+    """Load another build of the same C ABI (the stress build of build.build_stress); None = the product library."""
+    global _lib, LIB_PATH
+    _lib = None
+    LIB_PATH = path or os.path.join(_HERE, "librips_b200.so")
+    return lib()
+
+
 def _check(code, where):
     if code != RIPS_OK:
         raise RipsError(code, where)

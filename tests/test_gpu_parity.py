@@ -109,6 +109,36 @@ def test_sparse_path_randomized(R, seed):
     check_against_oracle(R, low, n, dim_max, thr, f"sparse seed {seed}: n={n} dim_max={dim_max} regime={regime} q={q}", mode="sparse")
 
 
+def test_stress_build(R):
+    """The chained scans (decoupled look-back of the sort, of compact mode, of the sparse path's scan, of the edge
+    ranking) and the lock-free reduction under shuffled schedules: the library built with -DRIPS_STRESS (sort tiles of
+    512 records instead of 5120, short chunks, pseudo-random delays in front of every publication) must produce the
+    same arrays.  compute-sanitizer is not available on this pool; this is the litmus test in its place."""
+    import torch
+    from paper_2003_07989_b200 import build
+    try:
+        R.use_library(build.build_stress())
+        rng = np.random.default_rng(5)
+        for n, lo, hi in [(513, 0, 8), (70001, 3, 19), (300007, 0, 24), (1 << 18, 40, 64)]:
+            a = rng.integers(0, 1 << 62, n, dtype=np.int64)
+            t = torch.from_numpy(a).cuda()
+            R.rips_sort_u64(t, lo, hi)
+            u = a.view(np.uint64)
+            key = (u >> np.uint64(lo)) & np.uint64((1 << (hi - lo)) - 1)
+            assert np.array_equal(t.cpu().numpy().view(np.uint64), u[np.argsort(key, kind="stable")]), (n, lo, hi)
+        for rep in range(3):
+            w = inputs.config(4, 200)
+            thr = float(np.float32(np.quantile(w.dist, 0.12)))
+            check_against_oracle(R, w.dist, w.n, 2, thr, "stress compact", mode="dense")
+            check_against_oracle(R, w.dist, w.n, 2, thr, "stress sparse", mode="sparse")
+            w = inputs.config(3, 70)
+            check_against_oracle(R, w.dist, w.n, 2, inf, "stress reduction")
+            w = inputs.config(2, 40)
+            check_against_oracle(R, w.dist, w.n, 3, inf, "stress slot")
+    finally:
+        R.use_library(None)
+
+
 def test_mode_is_fixed_by_the_first_stage1(R):
     w = inputs.config(1, 20)
     with R.Rips(w.dist, w.n, 1) as g:
