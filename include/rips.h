@@ -199,6 +199,19 @@ int rips_kernel_launches(rips_ctx* ctx, int64_t* launches);
  * sorted data ends in keys_dev.  stream as in rips_init. */
 int rips_sort_u64(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, int hi_bit, void* stream);
 
+/* The same sort for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): rips_sort_u64 allocates and frees its scratch (histograms, tickets, look-back status words) with
+ * cudaMalloc / cudaFree on every call; this entry point keeps that scratch in a static device array of 2 MiB inside the
+ * library (every GPU that loads the library holds it until the process exits) and calls no cudaMalloc, cudaFree or
+ * allocating library routine.  Same arguments, same result in keys_dev (tmp_dev = n more records, the caller's).
+ *   - n <= 4,194,304 records (2^22: what the array is sized for); more: RIPS_EINVAL, rips_last_error says so.
+ *   - Asynchronous: the work is enqueued on `stream` and the call returns; the result is valid once the stream has
+ *     been synchronised.
+ *   - The array is SHARED by every call on the device, whatever the stream or thread, and keeps the last call's
+ *     contents (the call clears what must start at zero): calls that overlap on the GPU race.  Serialise them -- one
+ *     stream, or an event between them. */
+int rips_sort_u64_static(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, int hi_bit, void* stream);
+
 const char* rips_strerror(int code);
 /* Text of the last CUDA error seen by this thread's calls ("" if none). */
 const char* rips_last_error(void);

@@ -5,6 +5,7 @@
 // in increasing combinatorial index leave each pass in increasing index within equal digits: the
 // index bits never have to be sorted.
 #include "radix_sort.cuh"
+#include <mutex>
 
 namespace {
 
@@ -339,6 +340,38 @@ SortPlan sort_make_plan(int lo_bit, int hi_bit)
 size_t sort_scratch_bytes(i64 n, const SortPlan& plan) { return scratch_layout(n, plan).total; }
 
 u64* sort_hist_ptr(void* scratch) { return (u64*)scratch; }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Static scratch for callers that cannot allocate (rips_sort_u64_static, include/rips.h): the sort's histograms,
+// tickets and look-back status words in a file-scope device array instead of a cudaMalloc'ed buffer.  Every GPU that
+// loads the library holds these RIPS_SORT_STATIC_BYTES until the process exits.  In HOST code the array's name is a
+// host-side stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, asked once
+// per device with that device current.  All calls share the array (it keeps the last call's contents: sort_u64 clears
+// the histograms, the tickets and, before every pass, the status words it is about to use), so calls that overlap on
+// the GPU race.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_sort_static_scratch[RIPS_SORT_STATIC_BYTES];
+
+cudaError_t sort_static_scratch(void** ptr, size_t* bytes)
+{
+    static std::mutex mu;
+    static void* addr[RIPS_SORT_STATIC_MAX_DEVICES] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= RIPS_SORT_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_sort_static_scratch); // the current device's copy of the array
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        addr[dev] = p;
+    }
+    *ptr = addr[dev];
+    *bytes = sizeof(g_sort_static_scratch);
+    return cudaSuccess;
+}
 
 cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream)
 {

@@ -1637,4 +1637,33 @@ int rips_sort_u64(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, 
     return RIPS_OK;
 }
 
+int rips_sort_u64_static(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, int hi_bit, void* stream)
+{
+    g_last_error.clear();
+    if (n < 0 || lo_bit < 0 || hi_bit > 64 || lo_bit >= hi_bit || (n > 0 && (!keys_dev || !tmp_dev))) return RIPS_EINVAL;
+    if (n > RIPS_SORT_STATIC_MAX_RECORDS) {
+        g_last_error = "rips_sort_u64_static: " + std::to_string(n) + " records exceed the maximum of " +
+                       std::to_string((long long)RIPS_SORT_STATIC_MAX_RECORDS) + " the static scratch is sized for (use rips_sort_u64)";
+        return RIPS_EINVAL;
+    }
+    if (n <= 1) return RIPS_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    SortPlan plan = sort_make_plan(lo_bit, hi_bit);
+    void* scratch = nullptr;
+    size_t bytes = 0;
+    cudaError_t e = sort_static_scratch(&scratch, &bytes);
+    if (e != cudaSuccess) return cuda_fail(e, "rips_sort_u64_static: address of the static scratch");
+    if (sort_scratch_bytes(n, plan) > bytes) { // (cannot happen in the product build: the maximum above is what the array holds)
+        g_last_error = "rips_sort_u64_static: " + std::to_string(n) + " records need " + std::to_string(sort_scratch_bytes(n, plan)) +
+                       " bytes of scratch, the static array holds " + std::to_string(bytes);
+        return RIPS_EINVAL;
+    }
+    u64* res = nullptr;
+    e = sort_u64(keys_dev, tmp_dev, n, plan, scratch, st, &res, nullptr, nullptr);
+    if (e == cudaSuccess && res != keys_dev)
+        e = cudaMemcpyAsync(keys_dev, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "rips_sort_u64_static");
+    return RIPS_OK;
+}
+
 } // extern "C"

@@ -22,7 +22,7 @@ SYMBOLS = [
     "rips_workspace_bytes", "rips_init", "rips_set_mode", "rips_compute", "rips_dim0", "rips_stage1", "rips_stage2", "rips_reduce", "rips_import_pivots",
     "rips_barcodes", "rips_filtration", "rips_apparent_pairs", "rips_nonapparent", "rips_pivots",
     "rips_pivot_lookup", "rips_stats", "rips_timings", "rips_device_bytes", "rips_workspace_in_use", "rips_kernel_launches",
-    "rips_sort_u64", "rips_strerror", "rips_last_error", "rips_last_required_bytes", "rips_free",
+    "rips_sort_u64", "rips_sort_u64_static", "rips_strerror", "rips_last_error", "rips_last_required_bytes", "rips_free",
 ]
 
 
@@ -86,6 +86,7 @@ def lib():
         l.rips_last_required_bytes.argtypes = []
         l.rips_last_required_bytes.restype = C.c_int64
         l.rips_sort_u64.argtypes = [vp, vp, i64, i32, i32, vp]
+        l.rips_sort_u64_static.argtypes = [vp, vp, i64, i32, i32, vp]
         l.rips_strerror.argtypes = [i32]
         l.rips_strerror.restype = C.c_char_p
         l.rips_last_error.argtypes = []
@@ -148,6 +149,17 @@ def rips_sort_u64(keys, lo_bit, hi_bit):
     tmp = torch.empty_like(keys)
     st = torch.cuda.current_stream().cuda_stream
     _check(lib().rips_sort_u64(keys.data_ptr(), tmp.data_ptr(), keys.numel(), lo_bit, hi_bit, st), "rips_sort_u64")
+    return keys
+
+
+def rips_sort_u64_static(keys, tmp, lo_bit, hi_bit):
+    """rips_sort_u64 without any allocation: the sort's scratch is a static array inside the library (at most 2^22
+    records), `tmp` is the caller's ping-pong buffer.  Enqueued on torch's current stream; calls must not overlap."""
+    torch = _torch()
+    assert keys.is_cuda and keys.dtype == torch.int64 and keys.is_contiguous()
+    assert tmp.is_cuda and tmp.dtype == torch.int64 and tmp.is_contiguous() and tmp.numel() >= keys.numel()
+    st = torch.cuda.current_stream().cuda_stream
+    _check(lib().rips_sort_u64_static(keys.data_ptr(), tmp.data_ptr(), keys.numel(), lo_bit, hi_bit, st), "rips_sort_u64_static")
     return keys
 
 
