@@ -141,6 +141,22 @@ def _compare_dimension(g, o, d, tag):
     assert st["n_essential"] == o[d]["essential"].size and st["n_reduced_pivots"] == o[d]["red_t"].size, tag
 
 
+def test_columns_with_more_than_2048_cofacets(R):
+    """2200 points, no threshold, dimension 1: every column has 2198 cofacets -- more than a warp's working column of
+    prereduce_kernel holds (2048 entries; round 1 wrote such columns off as zero columns) and more than the
+    shared-memory accumulator of reduce_kernel takes in one addition, so every non-apparent column goes through the
+    CTA-level reduction with coboundaries as runs of their own.  Every array against the oracle."""
+    w = inputs.config(1, 2200)
+    o = oracle.barcodes(w.dist, w.n, 1, w.threshold)
+    with R.Rips(w.dist, w.n, 1, w.threshold) as g:
+        g.compute()
+        for d in (0, 1):
+            _compare_dimension(g, o, d, f"{w.name} d={d}")
+        st = g.stats(1)
+        assert st["n_essential"] == 0 and st["n_reduce_serial"] == st["n_nonapparent"] == o[1]["non_cidx"].size
+        assert st["n_additions"] >= o[1]["additions"] > 0
+
+
 def test_config4_through_both_paths(R):
     """Config 4 (1000 points, threshold 0.15: 1.2 % of the edges) at full size through the sparse path (what
     RIPS_MODE_AUTO picks for it) and through the dense path: every array of every dimension against the oracle."""
