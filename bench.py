@@ -246,6 +246,8 @@ KERNELS = {  # rips_timings field -> kernel
 def algorithmic_bytes(field, st):
     """HBM bytes ONE launch of the kernel must move, from rips_stats of that dimension."""
     if field == "enumerate_ms":   # clearing bitmap read; one column record and one pair record written per slot
+        if st["n_removed_by_diameter"] > 0 and st["n_slots"] == st["n_columns"] + st["n_cleared"] and st["n_slots"] < st["n_candidates"]:
+            return 3 * RECORD_BYTES * st["n_slots"], 1    # sparse path: the simplex list read instead of a bitmap
         return st["n_candidates"] / 8 + 2 * RECORD_BYTES * st["n_slots"], 1
     if field == "sort_pass_ms":   # each pass reads and writes every record once
         return 2 * RECORD_BYTES * st["n_slots"], max(1, st["sort_passes"])
@@ -298,7 +300,10 @@ def run_b200(args):
     dev = host.cuda()
     wsize = rips.rips_workspace_bytes(w.n, D)
     free_b, _ = torch.cuda.mem_get_info()
-    workspace = torch.empty(min(wsize, int(free_b * 0.4)), dtype=torch.uint8, device="cuda")
+    if args.config == 3:      # the reduced columns of its dimension 1 fill in: 42 GB of arena
+        wsize = max(wsize, 72 << 30)
+    # (allocated before the resident context, whose own workspace grows with what its reduction needs)
+    workspace = torch.empty(min(wsize, int(free_b * 0.42)), dtype=torch.uint8, device="cuda")
 
     # ---- resident context; one full computation provides the clearing sets (and the barcode time)
     g = rips.Rips(dev, w.n, D, w.threshold)

@@ -150,6 +150,7 @@ struct DimState {
     bool caps_valid = false;      // a run of this dimension has fitted its lists: the sizes are known to suffice
     u64 irr_cap = 0, non_cap = 0; // capacities of the two small lists (records)
     int chunk_retry = 0, attempts = 0;
+    size_t arena_hint = 0;        // reduction: arena size to start from
     DevBuf simpA, simpB;          // sparse path: all simplices of this dimension within the threshold (vertex words)
     const u64* simp = nullptr;    // ... in increasing combinatorial index
     i64 n_simp = -1;
@@ -927,11 +928,15 @@ int run_reduce(rips_ctx* c, int d)
         RC(ensure(c, s.rd_rec, (size_t)nn * 8));
         RC(ensure(c, s.rd_rec2, (size_t)nn * 8));
         RC(ensure(c, s.rd_bars, (size_t)nn * 8));
+        // what follows the reduction is reserved before the arena is sized (the arena may take all that is left)
+        RC(ensure(c, s.red_t, (size_t)nn * 8));
+        RC(ensure(c, s.red_s, (size_t)nn * 8));
+        RC(ensure(c, c->sort_scratch2, sort_scratch_bytes(nn, sort_make_plan(jbits, jbits + s.tbits))));
         // the arena holds every reduced column and the working buffers; how much the columns fill in depends on
         // the input, so a run that exhausts it is repeated with a larger one
         // (library-owned workspace: a further chunk; caller's workspace: RIPS_ENOMEM with the size the next attempt
         // would have asked for).  First attempt: the largest free block of the workspace, at most 64 bytes per slot.
-        size_t arena_bytes = s.rd_arena.cap;
+        size_t arena_bytes = s.arena_hint; // (what the last reduction of this dimension used, plus a quarter)
         if (!arena_bytes) {
             const size_t want = std::max<size_t>((size_t)256 << 20, (size_t)s.slots * 64);
             const size_t have = c->pool.largest_free();
@@ -940,12 +945,18 @@ int run_reduce(rips_ctx* c, int d)
         }
         ReduceParams p;
         for (int attempt = 0;; ++attempt) {
+            // what the arena can be at most: after giving back the one it has, the largest free block of the workspace,
+            // or (library-owned workspace) a new chunk of 90 % of the device memory still free
             size_t limit = ~(size_t)0;
-            if (c->pool.may_grow) {
-                size_t free_b = 0, total_b = 0;
-                cudaMemGetInfo(&free_b, &total_b);
-                limit = s.rd_arena.cap + c->pool.largest_free() + (size_t)((double)free_b * 0.9);
-                if (arena_bytes > limit) arena_bytes = limit;
+            if (arena_bytes > s.rd_arena.cap) {
+                release(c, s.rd_arena);
+                limit = c->pool.largest_free();
+                if (c->pool.may_grow) {
+                    size_t free_b = 0, total_b = 0;
+                    cudaMemGetInfo(&free_b, &total_b);
+                    limit = std::max(limit, (size_t)((double)free_b * 0.9) & ~(size_t)255);
+                }
+                if (arena_bytes > limit && limit >= ((size_t)16 << 20)) arena_bytes = limit;
             }
             RC(ensure(c, s.rd_arena, arena_bytes));
             p.cols = s.non;
@@ -1000,6 +1011,7 @@ int run_reduce(rips_ctx* c, int d)
         s.stats.n_reduce_serial = (i64)c->h_counters[RDC_TODO];
         s.stats.n_reduce_displaced = (i64)c->h_counters[RDC_STEALS];
         s.stats.reduce_arena_bytes = (i64)c->h_counters[RDC_ARENA_TOP] * 8;
+        s.arena_hint = std::max<size_t>((size_t)16 << 20, ((size_t)s.stats.reduce_arena_bytes + (size_t)s.stats.reduce_arena_bytes / 4 + 255) & ~(size_t)255);
         // ---- second layer of the pair store as sorted arrays (t ascending), and the bars in column order
         CU(launch_pivot_records(p, jbits, (u64*)s.rd_rec.p, c->stream));
         SortPlan plan = sort_make_plan(jbits, jbits + s.tbits);
@@ -1024,6 +1036,7 @@ int run_reduce(rips_ctx* c, int d)
         const double t2 = now_ms();
         s.tim.reduce_device_ms = (float)(t1 - t0);
         s.tim.reduce_xfer_ms = (float)(t2 - t1);
+        release(c, s.rd_arena); // scratch of the reduction only: the next dimension may need the room
     } else {
         RC(ensure(c, s.red_t, 16));
         RC(ensure(c, s.red_s, 16));
