@@ -712,6 +712,9 @@ __device__ bool ws_merge_last_two(const ReduceParams& p, WorkSet& ws, u64* sm, R
     const i64 a = (i64)ws.len[k - 2] - ws.pos[k - 2], b = (i64)ws.len[k - 1] - ws.pos[k - 1];
     if (!ws_reserve(p, ws, 1, (u64)(a + b), sh)) return false;
     const i64 out = block_merge_xor(A, a, B, b, p.arena + ws.b_off, sm, sh);
+#ifdef RIPS_REDUCE_PROFILE
+    if (threadIdx.x == 0) atomicAdd((unsigned long long*)(p.counters + RDC_DBG + 5), (unsigned long long)((a + b + RD_TILE - 1) / RD_TILE));
+#endif
     __syncthreads();
     if (threadIdx.x == 0) ws.nruns = k - 2; // both inputs are gone: the stack ends below them
     __syncthreads();
@@ -784,6 +787,9 @@ __device__ bool acc_flush(const ReduceParams& p, WorkSet& ws, u64* sm, RdShared&
     __syncthreads();
     const int n = sh.acc_len - sh.acc_pos;
     if (n <= 0) return true;
+#ifdef RIPS_REDUCE_PROFILE
+    if (threadIdx.x == 0) atomicAdd((unsigned long long*)(p.counters + RDC_DBG + 5), 1ull << 40);
+#endif
     const u64* src = sh.acc[sh.acc_sel] + sh.acc_pos;
     if (!ws_push_copy(p, ws, src, n, sm, sh)) return false;
     if (threadIdx.x == 0) { sh.acc_pos = 0; sh.acc_len = 0; }
@@ -818,9 +824,12 @@ __device__ void ws_peek(WorkSet& ws, RdShared& sh)
         u64 h = is_acc ? (pos < len ? ptr[pos] : 0ull) : (act ? ws.head[lane] : 0ull);
         u64 m;
         for (;;) {
-            m = h;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(RIPS_FULL_MASK, m, o));
+            // the largest head: two 32-bit warp maxima (redux.sync) instead of a 64-bit butterfly of shuffles -- this loop
+            // runs once per consumed entry and is the longest part of an addition of a long chain
+            const u32 hh = (u32)(h >> 32);
+            const u32 mh = __reduce_max_sync(RIPS_FULL_MASK, hh);
+            const u32 ml = __reduce_max_sync(RIPS_FULL_MASK, hh == mh ? (u32)h : 0u);
+            m = ((u64)mh << 32) | (u64)ml;
             if (m == 0ull) break;
             const bool mine = (h == m);
             const u32 bal = __ballot_sync(RIPS_FULL_MASK, mine);

@@ -1003,9 +1003,10 @@ int run_reduce(rips_ctx* c, int d)
             return RIPS_ECUDA;
         }
 #ifdef RIPS_REDUCE_PROFILE
-        fprintf(stderr, "reduce d=%d: cycles summed over CTAs: peek %llu apparent %llu coboundary+sort %llu add %llu other-add %llu\n", d,
+        fprintf(stderr, "reduce d=%d: cycles summed over CTAs: peek %llu apparent %llu coboundary+sort %llu add %llu other-add %llu; flushes %llu merge tiles %llu\n", d,
                 (unsigned long long)c->h_counters[RDC_DBG], (unsigned long long)c->h_counters[RDC_DBG + 1], (unsigned long long)c->h_counters[RDC_DBG + 2],
-                (unsigned long long)c->h_counters[RDC_DBG + 3], (unsigned long long)c->h_counters[RDC_DBG + 4]);
+                (unsigned long long)c->h_counters[RDC_DBG + 3], (unsigned long long)c->h_counters[RDC_DBG + 4],
+                (unsigned long long)(c->h_counters[RDC_DBG + 5] >> 40), (unsigned long long)(c->h_counters[RDC_DBG + 5] & ((1ull << 40) - 1)));
 #endif
         n_adds = (i64)c->h_counters[RDC_ADDS];
         s.stats.n_reduce_serial = (i64)c->h_counters[RDC_TODO];
