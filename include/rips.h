@@ -201,7 +201,7 @@ int rips_sort_u64(uint64_t* keys_dev, uint64_t* tmp_dev, int64_t n, int lo_bit, 
 
 /* The same sort for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
  * forbid cudaMalloc): rips_sort_u64 allocates and frees its scratch (histograms, tickets, look-back status words) with
- * cudaMalloc / cudaFree on every call; this entry point keeps that scratch in a static device array of 2 MiB inside the
+ * cudaMalloc / cudaFree on every call; this entry point keeps that scratch in a static device array of 16 MiB inside the
  * library (every GPU that loads the library holds it until the process exits) and calls no cudaMalloc, cudaFree or
  * allocating library routine.  Same arguments, same result in keys_dev (tmp_dev = n more records, the caller's).
  *   - n <= 4,194,304 records (2^22: what the array is sized for); more: RIPS_EINVAL, rips_last_error says so.

@@ -92,10 +92,13 @@ struct Stage1Params {
 int stage1_chunk(u64 total, int compact, double est_survival, int retry, int sms);
 int stage1_stage_cap();
 cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t st);
-// bitmap |= bits of the given pivot rows t = (rows[i] >> shift) & mask, i < min(n_rows, *n_dev) (n_dev may be NULL);
-// records with (rows[i] >> sent_shift) == sent are skipped (sent_shift < 0: none)
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, const u64* n_dev, int shift, u64 mask, int sent_shift,
-                                u64 sent, cudaStream_t st);
+// the three sorted layers of dimension d-1's pivots, as the clearing bitmap's kernel reads them
+struct ClearLayers {
+    const u64* reg; i64 n_reg; int reg_tbits; u64 reg_mask, reg_sentinel;   // (v << tbits) | cidx(t); v == sentinel: no pair in this slot
+    const u64* irr; i64 n_irr; const u64* n_irr_dev; int irr_shift;         // (cidx(t) << shift) | j; count on the device (may be NULL)
+    const u64* red; i64 n_red;                                              // cidx(t)
+};
+cudaError_t launch_clear_bitmap(u32* bitmap, const ClearLayers& L, int sms, cudaStream_t st);
 
 // ------------------------------------------------------------------ sparse.cu (the sparse path, Algorithm 5)
 struct SparseExpand {

@@ -1,6 +1,6 @@
 // radix_sort.cu -- onesweep LSD radix sort of 64-bit records on a bit range, written by hand for
-// sm_100a (no CUB/Thrust).  One histogram kernel over all digits, then one kernel per digit that
-// ranks a tile in shared memory, resolves its global offsets with a decoupled look-back chained
+// sm_100a (no CUB/Thrust).  One histogram kernel over all digits (or a producer kernel that counts them while it
+// writes the records), then one kernel per digit that scans the digit's histogram, ranks a tile in shared memory, resolves its global offsets with a decoupled look-back chained
 // scan over (tile, bin) status words, and scatters coalesced runs.  Stable, so records that enter
 // in increasing combinatorial index leave each pass in increasing index within equal digits: the
 // index bits never have to be sorted.
@@ -73,28 +73,6 @@ __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const u64*
     }
 }
 
-// Exclusive scan over the bins of each digit, in place: hist[p][b] = number of records whose
-// digit p is smaller than b.  One block per pass.
-__global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64* hist)
-{
-    __shared__ u64 s_w[RIPS_SORT_MAX_BINS / 32];
-    u64* h = hist + (size_t)blockIdx.x * RIPS_SORT_MAX_BINS;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u64 c = h[tid];
-    u64 incl = c;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        u64 t = __shfl_up_sync(RIPS_FULL_MASK, incl, o);
-        if (lane >= o) incl += t;
-    }
-    if (lane == 31) s_w[warp] = incl;
-    __syncthreads();
-    u64 off = 0;
-#pragma unroll
-    for (int w = 0; w < RIPS_SORT_MAX_BINS / 32; ++w) off += (w < warp) ? s_w[w] : 0ull;
-    h[tid] = off + incl - c;
-}
-
 // ----------------------------------------------------------------------------------------------
 // One onesweep pass.  Per tile: (1) warp-striped coalesced load; (2) rank inside each warp with
 // match.any on the digit (one MATCH per record instead of a ballot per bit) and a per-warp
@@ -104,7 +82,7 @@ __global__ void __launch_bounds__(RIPS_SORT_MAX_BINS) sort_scan_bins_kernel(u64*
 // ----------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, const u64* __restrict__ n_dev, int shift, int bits,
-                     const u64* __restrict__ global_base, u64* status, u32* ticket, int pf_dist)
+                     const u64* __restrict__ hist_raw, u64* status, u32* ticket, int pf_dist)
 {
     if (n_dev) n = min(n, (i64)__ldg(n_dev)); // launched for the upper bound: the tiles past the count leave at once
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -116,13 +94,34 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, c
     u32* bin_start = whist + SORT_WARPS * RIPS_SORT_MAX_BINS;             // [MAX_BINS]
     __shared__ u32 s_tile;
     __shared__ u32 s_wsum[8];
+    __shared__ u64 s_gsum[RIPS_SORT_MAX_BINS / 32];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u); // tiles numbered in the order they start: every predecessor is resident or done
     u32* wh = whist + warp * RIPS_SORT_MAX_BINS;
 #pragma unroll
     for (int i = lane; i < RIPS_SORT_MAX_BINS; i += 32) wh[i] = 0;
+    // first slot of every bin in the output = exclusive scan of the digit's histogram (raw counts, complete before this
+    // pass starts), done by every tile for itself while its records are on their way: one kernel launch less per sort
+    // than a separate scan, and nothing of it lies on the tile's critical path
+    u64 g_cnt = 0, g_incl = 0;
+    if (tid < RIPS_SORT_MAX_BINS) {
+        g_cnt = __ldg(hist_raw + tid);
+        g_incl = g_cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u64 t = __shfl_up_sync(RIPS_FULL_MASK, g_incl, o);
+            if (lane >= o) g_incl += t;
+        }
+        if (lane == 31) s_gsum[warp] = g_incl;
+    }
     __syncthreads();
+    u64 g_base = 0; // records whose digit is smaller than `tid`
+    if (tid < RIPS_SORT_MAX_BINS) {
+#pragma unroll
+        for (int w = 0; w < RIPS_SORT_MAX_BINS / 32; ++w) g_base += (w < warp) ? s_gsum[w] : 0ull;
+        g_base += g_incl - g_cnt;
+    }
     const i64 tile = s_tile;
     const i64 base = tile * SORT_TILE;
     if (base >= n) return; // (uniform; only with a device-side count)
@@ -269,7 +268,7 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, c
             stress_jitter((u32)tile * 17u + (u32)tid);
             st_volatile_u64(status + tile * nbins + tid, LB_FLAG_INC | (excl + (u64)my_count));
         }
-        goff[tid] = __ldg(global_base + tid) + excl - (u64)bin_start[tid];
+        goff[tid] = g_base + excl - (u64)bin_start[tid];
     }
     __syncthreads();
 
@@ -296,7 +295,7 @@ size_t pass_smem_bytes(int)
 }
 
 struct ScratchLayout {
-    size_t hist_off, ticket_off, status_off, total;
+    size_t hist_off, ticket_off, status_off[RIPS_SORT_MAX_PASSES], total;
 };
 ScratchLayout scratch_layout(i64 n, const SortPlan& plan)
 {
@@ -304,12 +303,14 @@ ScratchLayout scratch_layout(i64 n, const SortPlan& plan)
     L.hist_off = 0;
     size_t hist_bytes = (size_t)RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 8;
     L.ticket_off = hist_bytes;
-    L.status_off = L.ticket_off + 256;
-    int maxbits = 1;
-    for (int p = 0; p < plan.npasses; ++p) maxbits = plan.bits[p] > maxbits ? plan.bits[p] : maxbits;
     i64 tiles = (n + SORT_TILE - 1) / SORT_TILE;
     if (tiles < 1) tiles = 1;
-    L.total = L.status_off + (size_t)tiles * ((size_t)1 << maxbits) * 8;
+    size_t at = L.ticket_off + 256;
+    for (int p = 0; p < RIPS_SORT_MAX_PASSES; ++p) { // every pass has its status words: one memset clears them all
+        L.status_off[p] = at;
+        if (p < plan.npasses) at += (size_t)tiles * ((size_t)1 << plan.bits[p]) * 8;
+    }
+    L.total = at;
     return L;
 }
 
@@ -373,9 +374,9 @@ cudaError_t sort_static_scratch(void** ptr, size_t* bytes)
     return cudaSuccess;
 }
 
-cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream)
+cudaError_t sort_prepare_fused(void* scratch, i64 n, const SortPlan& plan, cudaStream_t stream)
 {
-    return cudaMemsetAsync(scratch, 0, (size_t)RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 8 + 256, stream);
+    return cudaMemsetAsync(scratch, 0, scratch_layout(n, plan).total, stream);
 }
 
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream, u64** result,
@@ -411,11 +412,10 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     unsigned char* sc = (unsigned char*)scratch;
     u64* hist = (u64*)(sc + L.hist_off);
     u32* ticket = (u32*)(sc + L.ticket_off);
-    u64* status = (u64*)(sc + L.status_off);
     const i64 tiles = (n + SORT_TILE - 1) / SORT_TILE;
 
     cudaError_t e = cudaSuccess;
-    if (!hist_ready) e = cudaMemsetAsync(sc, 0, L.status_off, stream); // else sort_prepare_fused did it before the producer ran
+    if (!hist_ready) e = cudaMemsetAsync(sc, 0, L.total, stream); // histograms, tickets, status words of every pass (else sort_prepare_fused did it before the producer ran)
     if (e != cudaSuccess) return e;
     PlanDev pd;
     pd.npasses = plan.npasses;
@@ -428,18 +428,13 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
             sort_histogram_kernel<<<(unsigned)blocks, HIST_THREADS, plan.npasses * RIPS_SORT_MAX_BINS * 4, stream>>>(a, n, n_dev, pd, hist);
             if (launches) *launches += 1;
         }
-        sort_scan_bins_kernel<<<plan.npasses, RIPS_SORT_MAX_BINS, 0, stream>>>(hist);
-        if (launches) *launches += 1;
     }
     rec(1);
     u64* src = a;
     u64* dst = b;
     for (int p = 0; p < plan.npasses; ++p) {
-        size_t status_bytes = (size_t)tiles * ((size_t)1 << plan.bits[p]) * 8;
-        e = cudaMemsetAsync(status, 0, status_bytes, stream);
-        if (e != cudaSuccess) return e;
         onesweep_pass_kernel<<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-            src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, status, ticket + p, pf_dist);
+            src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, (u64*)(sc + L.status_off[p]), ticket + p, pf_dist);
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }

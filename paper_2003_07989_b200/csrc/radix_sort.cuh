@@ -38,11 +38,12 @@ struct SortTimes {
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
                      u64** result, SortTimes* times, i64* launches, bool hist_ready = false,
                      bool skewed_digits = false, const u64* n_dev = nullptr);
-cudaError_t sort_prepare_fused(void* scratch, cudaStream_t stream);
+// (clears the whole scratch of a sort of n records: histograms, tickets, the status words of every pass)
+cudaError_t sort_prepare_fused(void* scratch, i64 n, const SortPlan& plan, cudaStream_t stream);
 
 // The sort's scratch as a static device array (radix_sort.cu): its device address on the CURRENT device and its size.
 // No allocation; the address is asked for once per device.  Shared by every caller: see the note at the array.
-#define RIPS_SORT_STATIC_BYTES (2u << 20)
+#define RIPS_SORT_STATIC_BYTES (16u << 20)
 #define RIPS_SORT_STATIC_MAX_RECORDS (1ll << 22)
 #define RIPS_SORT_STATIC_MAX_DEVICES 64
 cudaError_t sort_static_scratch(void** ptr, size_t* bytes);

@@ -668,15 +668,21 @@ int run_stage1(rips_ctx* c, int d)
         RC(ensure(c, s.bitmap, (size_t)words * 4));
         CU(cudaMemsetAsync(s.bitmap.p, 0, (size_t)words * 4, c->stream));
         const u64 pmask = (prev.tbits >= 64) ? ~0ull : ((1ull << prev.tbits) - 1ull);
-        // regular pairs: every slot of the partitioned pair array, the sentinels (cofacet vertex = n) skipped;
-        // irregular pairs: as many as the previous dimension's kernel counted (on the device)
-        if (d >= 2 && prev.reg)
-            CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.reg, prev.slots, nullptr, 0, pmask, prev.tbits, (u64)n, c->stream));
-        if (d >= 2 && prev.irr)
-            CU(launch_clear_bitmap((u32*)s.bitmap.p, prev.irr, (i64)prev.irr_cap, (const u64*)prev.d_cnt.p + S1C_IRREGULAR,
-                                   RIPS_PAIR_POS_BITS, ~0ull, -1, 0, c->stream));
-        CU(launch_clear_bitmap((u32*)s.bitmap.p, (const u64*)prev.red_t.p, prev.n_red, nullptr, 0, ~0ull, -1, 0, c->stream));
-        c->launches += (d >= 2 && prev.reg && prev.slots > 0) + (d >= 2 && prev.irr && prev.irr_cap > 0) + (prev.n_red > 0);
+        ClearLayers L;
+        const bool lower = d >= 2;
+        L.reg = (lower && prev.reg) ? prev.reg : nullptr;
+        L.n_reg = L.reg ? prev.slots : 0;
+        L.reg_tbits = prev.tbits;
+        L.reg_mask = pmask;
+        L.reg_sentinel = (u64)n;
+        L.irr = (lower && prev.irr) ? prev.irr : nullptr;
+        L.n_irr = L.irr ? (i64)prev.irr_cap : 0;
+        L.n_irr_dev = L.irr ? (const u64*)prev.d_cnt.p + S1C_IRREGULAR : nullptr;
+        L.irr_shift = RIPS_PAIR_POS_BITS;
+        L.red = (const u64*)prev.red_t.p;
+        L.n_red = prev.n_red;
+        CU(launch_clear_bitmap((u32*)s.bitmap.p, L, c->sms, c->stream));
+        c->launches += (L.n_reg > 0 || L.n_irr > 0 || L.n_red > 0);
         cs.bitmap = (const u32*)s.bitmap.p;
     } else if (d >= 2) {
         // no bitmap: the kernel searches the sorted layers, which needs their sizes on the host
@@ -767,13 +773,13 @@ int run_stage1(rips_ctx* c, int d)
     CU(cudaMemsetAsync(d_cnt, 0, 128, c->stream));
     if (s.compact) CU(cudaMemsetAsync(s.s1_status.p, 0, (size_t)tiles * 8, c->stream));
     if (fused) {
-        CU(sort_prepare_fused(c->sort_scratch.p, c->stream));
+        CU(sort_prepare_fused(c->sort_scratch.p, (i64)cap, plan, c->stream));
         p.fh_cols.hist = sort_hist_ptr(c->sort_scratch.p);
         p.fh_cols.npasses = plan.npasses;
         for (int r = 0; r < plan.npasses; ++r) { p.fh_cols.shift[r] = plan.shift[r]; p.fh_cols.bits[r] = plan.bits[r]; }
     }
     if (s.pair_fused) {
-        CU(sort_prepare_fused(s.pair_scratch.p, c->stream));
+        CU(sort_prepare_fused(s.pair_scratch.p, (i64)cap, s.pair_plan, c->stream));
         p.fh_pairs.hist = sort_hist_ptr(s.pair_scratch.p);
         p.fh_pairs.npasses = s.pair_plan.npasses;
         for (int r = 0; r < s.pair_plan.npasses; ++r) {
@@ -1167,7 +1173,8 @@ long double dim_bytes(long double cand, long double keep)
 {
     const long double slots = std::max<long double>(4096.0L, cand * keep);
     const long double lists = std::max<long double>(4096.0L, slots / 8);
-    return slots * 32 + lists * 8 * 4 + cand / 8 + 64 + 3 * ((slots / 5120 + 2) * 2048 + (1 << 15)) + slots * (12 + 16 + 16) + lists * 12 +
+    return slots * 32 + lists * 8 * 4 + cand / 8 + 64 + 8 * ((slots / 5120 + 2) * 2048) + 16 * ((lists / 5120 + 2) * 2048) + 5 * (1 << 15) +
+           slots * (12 + 16 + 16) + lists * 12 +
            lists * 96 + std::max<long double>((long double)(256u << 20), slots * 64);
 }
 

@@ -21,6 +21,8 @@
 //     coalesced stores.  With a threshold survivors are compacted in increasing index with a
 //     warp-level decoupled look-back.
 //   * the digit histograms of the two sorts that follow are accumulated on the way out.
+#include <algorithm>
+
 #include "apparent.cuh"
 #include "kernels.cuh"
 
@@ -731,16 +733,27 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
     }
 }
 
-// bitmap |= bits of the rows t = (rows[i] >> shift) & mask, i < min(n_rows, *n_dev); a record whose field above
-// `sent_shift` equals `sent` is a sentinel (the slot of a column with no regular pair) and is skipped
-__global__ void clear_bitmap_kernel(u32* bitmap, const u64* __restrict__ rows, i64 n_rows, const u64* __restrict__ n_dev, int shift,
-                                    u64 mask, int sent_shift, u64 sent)
+// bitmap |= bits of the pivot rows of the three layers of dimension d-1's pair store, in one launch (grid-stride over
+// the three segments one after the other).  Regular layer: every slot of the partitioned pair array, the sentinels
+// (cofacet vertex = n) skipped; irregular layer: as many records as the fused kernel of dimension d-1 counted (the
+// count lives on the device); reduced layer: plain row indices.
+__global__ void clear_bitmap_kernel(u32* bitmap, const ClearLayers L)
 {
-    if (n_dev) n_rows = min(n_rows, (i64)__ldg(n_dev));
-    for (i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows; i += (i64)gridDim.x * blockDim.x) {
-        const u64 r = __ldg(rows + i);
-        if (sent_shift >= 0 && (r >> sent_shift) == sent) continue;
-        const u64 t = (r >> shift) & mask;
+    const i64 stride = (i64)gridDim.x * blockDim.x, t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    for (i64 i = t0; i < L.n_reg; i += stride) {
+        const u64 r = __ldg(L.reg + i);
+        if ((r >> L.reg_tbits) == L.reg_sentinel) continue;
+        const u64 t = r & L.reg_mask;
+        atomicOr(bitmap + (t >> 5), 1u << (t & 31));
+    }
+    i64 n_irr = L.n_irr;
+    if (L.n_irr_dev) n_irr = min(n_irr, (i64)__ldg(L.n_irr_dev));
+    for (i64 i = t0; i < n_irr; i += stride) {
+        const u64 t = __ldg(L.irr + i) >> L.irr_shift;
+        atomicOr(bitmap + (t >> 5), 1u << (t & 31));
+    }
+    for (i64 i = t0; i < L.n_red; i += stride) {
+        const u64 t = __ldg(L.red + i);
         atomicOr(bitmap + (t >> 5), 1u << (t & 31));
     }
 }
@@ -822,12 +835,12 @@ cudaError_t launch_stage1(int M, int kf_u16, const Stage1Params& p, cudaStream_t
 #undef S1_CASE
 }
 
-cudaError_t launch_clear_bitmap(u32* bitmap, const u64* rows, i64 n_rows, const u64* n_dev, int shift, u64 mask, int sent_shift,
-                                u64 sent, cudaStream_t st)
+cudaError_t launch_clear_bitmap(u32* bitmap, const ClearLayers& L, int sms, cudaStream_t st)
 {
-    if (n_rows == 0) return cudaSuccess;
-    i64 blocks = (n_rows + 255) / 256;
-    if (blocks > 148 * 64) blocks = 148 * 64;
-    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, rows, n_rows, n_dev, shift, mask, sent_shift, sent);
+    const i64 n = std::max(L.n_reg, std::max(L.n_irr, L.n_red));
+    if (n == 0) return cudaSuccess;
+    i64 blocks = (n + 255) / 256;
+    if (blocks > (i64)sms * 16) blocks = (i64)sms * 16;
+    clear_bitmap_kernel<<<(unsigned)blocks, 256, 0, st>>>(bitmap, L);
     return cudaGetLastError();
 }
