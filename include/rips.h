@@ -92,11 +92,11 @@ typedef struct {
 typedef struct {
     float clear_bitmap_ms;   /* a4: clearing bitmap built from P_{d-1} */
     float enumerate_ms;      /* a3-a5 + a7: the fused kernel (enumerate, diameter, filter, slot/compaction, apparent test) */
-    float sort_hist_ms;      /* a6: digit histograms */
+    float sort_hist_ms;      /* a6: digit histograms (~0 when the fused kernel accumulated them) */
     float sort_pass_ms;      /* a6: all onesweep passes */
     float apparent_ms;       /* a8: full sorts of the two small lists (irregular pairs, non-apparent columns), on side
                                 streams beside the fused kernel's successors */
-    float pair_hist_ms;      /* a9: bin scan (the histogram itself is accumulated by the fused kernel) */
+    float pair_hist_ms;      /* a9: ~0 (the histogram is accumulated by the fused kernel, its scan runs inside the pass kernel) */
     float pair_sort_ms;      /* a9: stable partition of the pair slots by cofacet vertex (onesweep passes) */
     float stage1_ms;         /* whole stage 1 as enqueued (including memsets, scalar read-back) */
     float stage2_ms;         /* whole stage 2: from its first launch (beside stage 1's sort) to the join on the main stream */
