@@ -39,7 +39,7 @@ STRESS_FLAGS = ["-DRIPS_STRESS", "-DRIPS_SORT_THREADS=256", "-DRIPS_SORT_IPT=2",
 
 def _compile(out: str, extra, verbose: bool) -> None:
     tmp = out + f".{os.getpid()}.tmp"
-    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+    cmd = [nvcc(), "--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC,-O3", "-Xcompiler", "-Wall"] + list(extra) + \
           ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
     if verbose:
@@ -47,6 +47,14 @@ def _compile(out: str, extra, verbose: bool) -> None:
         cmd.insert(2, "-v")
     subprocess.check_call(cmd)
     os.replace(tmp, out)
+
+
+def build_all(force: bool = False) -> None:
+    """The product library and the stress variant, compiled side by side."""
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=2) as ex:
+        a, b = ex.submit(build, force), ex.submit(build_stress, force)
+        a.result(); b.result()
 
 
 def _stale(out: str) -> bool:
