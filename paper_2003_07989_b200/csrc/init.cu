@@ -103,7 +103,32 @@ __global__ void build_full_keys_kernel(const u32* __restrict__ K, int n, int pit
     Kf[(size_t)i * pitch + j] = (KT)x;
 }
 
+// Sf[i*spitch + b] = max of Kf[i][32b .. 32b+31]: the largest key+1 (the shortest edge) from vertex i into block b of 32
+// vertices.  The fused kernels' warp scan for a cofacet of equal diameter reads these block maxima first and skips
+// every block that cannot hold one (stage1.cu, summary_scan).  One warp per (row, block).
+template <typename KT>
+__global__ void build_block_max_kernel(const KT* __restrict__ Kf, int n, int pitch, KT* __restrict__ Sf, int spitch, int nb)
+{
+    const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), i = blockIdx.y, lane = threadIdx.x & 31;
+    if (b >= nb) return;
+    const int j = b * 32 + lane;
+    u32 x = 0;
+    if (j < n) x = (u32)Kf[(size_t)i * pitch + j];
+    x = __reduce_max_sync(RIPS_FULL_MASK, x);
+    if (lane == 0) Sf[(size_t)i * spitch + b] = (KT)x;
+}
+
 } // namespace
+
+cudaError_t launch_build_block_max(const void* Kf, int n, int pitch, void* Sf, int spitch, int kf_u16, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    const int nb = (n + 31) / 32;
+    dim3 g((unsigned)((nb + 7) / 8), (unsigned)n);
+    if (kf_u16) build_block_max_kernel<unsigned short><<<g, 256, 0, st>>>((const unsigned short*)Kf, n, pitch, (unsigned short*)Sf, spitch, nb);
+    else build_block_max_kernel<u32><<<g, 256, 0, st>>>((const u32*)Kf, n, pitch, (u32*)Sf, spitch, nb);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_build_full_keys(const u32* K, int n, int pitch, void* Kf, int kf_u16, cudaStream_t st)
 {

@@ -32,6 +32,14 @@ cudaError_t launch_rank_edges(const u64* rec_sorted, i64 E, u32* K, float* value
 i64 rank_edges_tiles(i64 E);
 // Kf (see common.cuh) from K: n*n entries of u16 (kf_u16 != 0) or u32
 cudaError_t launch_build_full_keys(const u32* K, int n, int pitch, void* Kf, int kf_u16, cudaStream_t st);
+// Sf[i*spitch + b] = max of Kf[i][32b .. 32b+31] (same entry type as Kf); spitch >= ceil(n / 32).  Built by rips_init
+// from SUMMARY_MIN_N points on: below that a scan of all vertices is a few warp steps and the table buys nothing.
+#ifdef RIPS_STRESS
+constexpr int SUMMARY_MIN_N = 8;     // the small inputs of the stress tests take the summary-guided scan too
+#else
+constexpr int SUMMARY_MIN_N = 2048;
+#endif
+cudaError_t launch_build_block_max(const void* Kf, int n, int pitch, void* Sf, int spitch, int kf_u16, cudaStream_t st);
 
 // ------------------------------------------------------------------ dim0.cu
 struct Dim0Out {
@@ -63,6 +71,8 @@ enum { S1C_KEPT = 0, S1C_OVER = 1, S1C_CLEARED = 2, S1C_REGULAR = 3, S1C_IRREGUL
 struct Stage1Params {
     const void* Kf;   // full key matrix (u16 or u32, see launch_stage1's kf_u16), row pitch `pitch` entries
     int pitch;
+    const void* Sf;   // block maxima of Kf's rows (launch_build_block_max), or NULL: the warp scan then reads every vertex
+    int spitch;
     BinomTable bt;
     int n;
     u64 total;        // C(n, d+1)

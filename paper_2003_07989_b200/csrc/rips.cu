@@ -204,6 +204,8 @@ struct rips_ctx {
     u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
     u32* d_K = nullptr;
     void* d_Kf = nullptr;  // full symmetric matrix of key+1 (common.cuh)
+    void* d_Sf = nullptr;  // block maxima of its rows (n >= SUMMARY_MIN_N; kernels.cuh), else NULL
+    int sf_pitch = 0;
     int kf_u16 = 0, kf_pitch = 1, vbits = 1;
     int sms = 148;       // multiprocessors of the device
     bool use_graphs = true;  // switched off for the context if a capture fails
@@ -227,7 +229,7 @@ struct rips_ctx {
     DevBuf d0_pairs, d0_death, d0_uf;
     std::vector<DimState> dims; // index d, 0 .. dim_max+1
     Pool pool;
-    DevBuf b_dist, b_edges, b_K, b_Kf, b_values, b_binom, b_counters, b_tickets, b_init_tmp, b_init_status;
+    DevBuf b_dist, b_edges, b_K, b_Kf, b_Sf, b_values, b_binom, b_counters, b_tickets, b_init_tmp, b_init_status;
     i64 launches = 0;
     BinomTable bt() const { return BinomTable{d_binom, (int)(n + 1)}; }
 };
@@ -707,6 +709,8 @@ int run_stage1(rips_ctx* c, int d)
     Stage1Params p;
     p.Kf = c->d_Kf;
     p.pitch = c->kf_pitch;
+    p.Sf = c->d_Sf;
+    p.spitch = c->sf_pitch;
     p.bt = c->bt();
     p.n = (int)n;
     p.total = s.total;
@@ -1139,6 +1143,13 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         CU(cudaMemsetAsync(c->d_Kf, 0, kf_bytes, c->stream));
         CU(launch_build_full_keys(c->d_K, (int)n, pitch, c->d_Kf, c->kf_u16, c->stream));
         c->launches += 1;
+        if (n >= SUMMARY_MIN_N) {
+            c->sf_pitch = (int)((n + 31) / 32);
+            RC(ensure(c, c->b_Sf, (size_t)n * (size_t)c->sf_pitch * (c->kf_u16 ? 2 : 4)));
+            c->d_Sf = c->b_Sf.p;
+            CU(launch_build_block_max(c->d_Kf, (int)n, pitch, c->d_Sf, c->sf_pitch, c->kf_u16, c->stream));
+            c->launches += 1;
+        }
         c->vbits = bits_for((u64)(n - 1));
     }
     // keys are ranks in descending value order: thr_key = number of distinct values above the threshold
@@ -1159,7 +1170,8 @@ size_t setup_bytes(i64 n, int kmax)
 {
     const size_t E = (size_t)(n * (n - 1) / 2) + 1;
     SortPlan plan = sort_make_plan(32, 64);
-    return E * (4 + 8 + 8 + 4 + 4) + (size_t)n * (size_t)(n + 4) * 4 + (size_t)(kmax + 1) * (size_t)(n + 1) * 8 + sort_scratch_bytes((i64)E, plan) +
+    return E * (4 + 8 + 8 + 4 + 4) + (size_t)n * (size_t)(n + 4) * 4 + (n >= SUMMARY_MIN_N ? (size_t)n * (size_t)(n / 32 + 2) * 4 : 0) +
+           (size_t)(kmax + 1) * (size_t)(n + 1) * 8 + sort_scratch_bytes((i64)E, plan) +
            (E / 2048 + 1) * 8 + (size_t)n * 20 + (1 << 16);
 }
 

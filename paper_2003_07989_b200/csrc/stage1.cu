@@ -64,6 +64,54 @@ struct BlockHists {
     u32 pmk[S1_MAX_FUSED_P];
 };
 
+// The warp's scan of the cofacet vertices base, base-1, ..., 0 of one simplex (rows Kf + xs and Kf + v1s of its two
+// lowest vertices xq < v1q; `extra(v)` is the part of the test its other vertices contribute), guided by the block
+// maxima Sf (init.cu, build_block_max_kernel): lane l reads the maxima of block bt - l of both rows, and only blocks
+// whose maximum reaches ks in BOTH rows are read vertex by vertex, four blocks per round (their loads independent),
+// from the top.  Returns the largest vertex <= base | 31 that passes, or -1.  Vertices above `base` in the first block
+// were tested by the caller and fail again.  With keys of a random matrix a column without such a cofacet costs
+// n / 512 coalesced loads instead of n / 16: the scan of all n vertices is what binds the fused kernel when n is in
+// the thousands (Section 6.6's workload).  Every lane of the warp must call it with the same arguments.
+template <typename KT, typename EX>
+__device__ __forceinline__ int summary_scan(const KT* __restrict__ Kf, const KT* __restrict__ Sf, const int spitch, const int n,
+                                            const int xs, const int v1s, const int xq, const int v1q, const u32 ks, const int base,
+                                            const int lane, EX extra)
+{
+    int res = -1;
+    const KT* __restrict__ sx = Sf + (size_t)xq * spitch;
+    const KT* __restrict__ s1 = Sf + (size_t)v1q * spitch;
+    for (int bt = base >> 5; bt >= 0 && res < 0; bt -= 32) {
+        const int b = bt - lane;
+        u32 s = 0u;
+        if (b >= 0) s = min((u32)__ldg(sx + b), (u32)__ldg(s1 + b));
+        u32 cand = __ballot_sync(RIPS_FULL_MASK, s >= ks);
+        while (cand && res < 0) {
+            int blk[4];
+            u32 mm[4];
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                blk[g] = -1;
+                if (cand) {
+                    blk[g] = bt - (__ffs(cand) - 1);
+                    cand &= cand - 1;
+                }
+            }
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                const int vv = blk[g] * 32 + 31 - lane;
+                mm[g] = 0u;
+                if (blk[g] >= 0 && vv < n) mm[g] = min(min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]), extra(vv));
+            }
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                const u32 bb = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
+                if (bb && res < 0) res = blk[g] * 32 + 31 - (__ffs(bb) - 1);
+            }
+        }
+    }
+    return res;
+}
+
 // KS: the key matrix is staged in shared memory.  A template parameter, not a run-time flag, so that the
 // compiler addresses Kf with 32-bit shared-memory addresses (LDS) instead of generic 64-bit ones: the
 // kernel is bound by instruction issue, and address arithmetic is a large part of its instructions.
@@ -243,6 +291,16 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
                         }
                         const u32 b = __ballot_sync(RIPS_FULL_MASK, ok);
                         if (b) { res = base - (__ffs(b) - 1); break; }
+                        if (p.Sf) { // the rest guided by the block maxima of the two rows
+                            res = summary_scan<KT>(Kf, reinterpret_cast<const KT*>(p.Sf), p.spitch, n, xs * pitch, v1s * pitch, xs, v1s, ks,
+                                                   base - 32, lane, [&](const int w) {
+                                                       u32 m2 = 0xffffffffu;
+#pragma unroll
+                                                       for (int j = 2; j < M; ++j) m2 = min(m2, (u32)Kf[v[j] * pitch + w]);
+                                                       return m2;
+                                                   });
+                            break;
+                        }
                     }
                     if (lane == src) fv = res;
                 }
@@ -441,8 +499,8 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
 //   * nothing is counted per warp step: the number of columns is total - over - cleared.
 // Same records, same lists, same counters as enumerate_apparent_kernel (the tests compare both with the oracle).
 // ---------------------------------------------------------------------------------------------------------------
-template <int M, typename KT, bool KS>
-__global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1Params p)
+template <int M, typename KT, bool KS, bool SUM>
+__global__ void __launch_bounds__(S1_THREADS, SUM ? 2 : 0) enumerate_slot_kernel(const Stage1Params p)
 {
     extern __shared__ __align__(16) unsigned char smem1[];
     __shared__ u32 s_hist_cols[S1_MAX_FUSED][256];
@@ -465,8 +523,10 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
         Kf = reinterpret_cast<const KT*>(p.Kf);
     }
     u64* const sprec = reinterpret_cast<u64*>(smem1 + off_b); // record of a regular pair with cofacet vertex v, minus cidx(s)
-    for (int i = tid; i < n; i += S1_THREADS) sprec[i] = ((u64)(u32)i << p.tbits) + p.bt(i, M + 1);
-    off_b += (size_t)n * 8;
+    if (!SUM) { // (SUM: thousands of points, where this table would cost the second resident block; C(v, M+1) is read from HBM's copy)
+        for (int i = tid; i < n; i += S1_THREADS) sprec[i] = ((u64)(u32)i << p.tbits) + p.bt(i, M + 1);
+        off_b += (size_t)n * 8;
+    }
     KT* const u2 = reinterpret_cast<KT*>(smem1 + off_b) + (size_t)warp * ((n + 7) & ~7);
     for (int i = tid; i < S1_MAX_FUSED * 256; i += S1_THREADS) (&s_hist_cols[0][0])[i] = 0;
     for (int i = tid; i < S1_MAX_FUSED_P * 256; i += S1_THREADS) (&s_hist_pairs[0][0])[i] = 0;
@@ -605,6 +665,14 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
                             if (bb) res = base - (__ffs(bb) - 1);
                             base -= 32;
                         }
+                        if (SUM) { // (the block maxima of the two rows say which blocks of 32 vertices are worth reading)
+                            const int xq = __shfl_sync(RIPS_FULL_MASK, lx, src);
+                            const int v1q = __shfl_sync(RIPS_FULL_MASK, lv1, src);
+                            if (res < 0)
+                                res = summary_scan<KT>(Kf, reinterpret_cast<const KT*>(p.Sf), p.spitch, n, xs, v1s, xq, v1q, ks, base, lane,
+                                                       [&](const int w) { return (M > 2) ? (u32)u2[w] : 0xffffffffu; });
+                            base = -1;
+                        }
                         for (; base >= 0 && res < 0; base -= 128) {
                             u32 mm[4];
 #pragma unroll
@@ -632,7 +700,7 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_slot_kernel(const Stage1
                 const u32 fvv = regular ? (u32)fv : (u32)n;
                 u64 prec = psentinel;
                 if (regular) {
-                    prec = ci + sprec[fv];
+                    prec = SUM ? ci + ((u64)(u32)fv << p.tbits) + p.bt(fv, M + 1) : ci + sprec[fv];
                     ++n_reg;
                 }
                 u64 rec = (u64)kk << lowbits;
@@ -782,9 +850,11 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
     const bool kf_fits = kf_bytes <= S1_KF_SMEM_LIMIT;
     if (!p.compact && !p.count_only) {
         // slot mode: the leaner kernel, if its tables fit (C(., M+1) and one row of U2 per warp)
-        const size_t tables = (size_t)p.n * 8 + (M > 2 ? (size_t)S1_WARPS * ((p.n + 7) & ~7) * sizeof(KT) : 0);
-        if (kf_fits && kf_bytes + tables <= 190 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, true>, p, kf_bytes + tables, st);
-        if (tables <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false>, p, tables, st);
+        const size_t u2rows = M > 2 ? (size_t)S1_WARPS * ((p.n + 7) & ~7) * sizeof(KT) : 0;
+        const size_t tables = (size_t)p.n * 8 + u2rows;
+        if (p.Sf && u2rows <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, true>, p, u2rows, st);
+        if (kf_fits && kf_bytes + tables <= 190 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, true, false>, p, kf_bytes + tables, st);
+        if (tables <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, false>, p, tables, st);
     }
     const int k_in = (!p.compact && !p.count_only && kf_fits) ? 1 : 0;
     const size_t smem = (k_in ? kf_bytes : 0) +

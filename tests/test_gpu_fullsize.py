@@ -157,6 +157,26 @@ def test_columns_with_more_than_2048_cofacets(R):
         assert st["n_additions"] >= o[1]["additions"] > 0
 
 
+def test_block_maxima_guide_the_scan_in_both_fused_kernels(R):
+    """From 2048 points on rips_init builds the block maxima of the key matrix's rows and the fused kernels' warp scan
+    for a cofacet of equal diameter reads only the blocks of 32 vertices they leave open (stage1.cu, summary_scan).
+    2300 points in dimension 1: without a threshold (slot mode, enumerate_slot_kernel) and with one that admits 40 %
+    of the edges (compact mode, enumerate_apparent_kernel), the dense path forced.  Every array against the oracle."""
+    w = inputs.config(1, 2300)
+    thr = float(np.quantile(w.dist, 0.4))
+    for threshold in (w.threshold, thr):
+        o = oracle.barcodes(w.dist, w.n, 1, threshold)
+        with R.Rips(w.dist, w.n, 1, threshold) as g:
+            g.set_mode("dense")
+            g.compute()
+            for d in (0, 1):
+                _compare_dimension(g, o, d, f"{w.name} thr={threshold} d={d}")
+            st = g.stats(1)
+            assert st["n_candidates"] == comb(w.n, 2)
+            if threshold == thr:
+                assert 0.39 * comb(w.n, 2) < st["n_columns"] + st["n_cleared"] < 0.41 * comb(w.n, 2)
+
+
 def test_config4_through_both_paths(R):
     """Config 4 (1000 points, threshold 0.15: 1.2 % of the edges) at full size through the sparse path (what
     RIPS_MODE_AUTO picks for it) and through the dense path: every array of every dimension against the oracle."""
