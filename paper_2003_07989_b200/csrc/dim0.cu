@@ -4,7 +4,8 @@
 // ascending) read backwards ARE the filtration order of the 1-simplices (diameter ascending,
 // cidx descending).  Each round 1024 threads test 1024 edges against the current
 // forest in parallel (read-mostly finds with path compression); the few edges whose endpoints are
-// still in different components are compacted in order and merged serially by one thread, which
+// still in different components are compacted in order -- record and vertices into shared memory, so that
+// no load from HBM sits on the serial path -- and merged serially by one thread, which
 // is what makes the result independent of scheduling.  The loop stops after n-1 merges.
 #include "kernels.cuh"
 
@@ -39,7 +40,8 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
 {
     extern __shared__ u32 s_uf[];
     if (SM) parent_maxv = s_uf;
-    __shared__ u32 s_list[D0_THREADS];
+    __shared__ u64 s_rec[D0_THREADS];  // the round's surviving edges in filtration order: record,
+    __shared__ u32 s_ab[D0_THREADS];   // vertices (a << 16) | b (n <= 46340)
     __shared__ u32 s_wcount[D0_THREADS / 32];
     __shared__ i64 s_start;
     __shared__ u32 s_merges;
@@ -63,10 +65,12 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
     for (i64 hi = E; hi > start; hi -= D0_THREADS) {
         const i64 i = hi - 1 - tid;
         bool cand = false;
+        u64 r_mine = 0;
+        int a_mine = 0, b_mine = 0;
         if (i >= start) {
-            int a, b;
-            edge_vertices((u32)rec[i], &a, &b);
-            cand = find_root(parent, a) != find_root(parent, b);
+            r_mine = rec[i];
+            edge_vertices((u32)r_mine, &a_mine, &b_mine);
+            cand = find_root(parent, a_mine) != find_root(parent, b_mine);
         }
         const u32 bal = __ballot_sync(RIPS_FULL_MASK, cand);
         if (lane == 0) s_wcount[warp] = __popc(bal);
@@ -77,15 +81,18 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
             if (w < warp) off += c;
             tot += c;
         }
-        if (cand) s_list[off + __popc(bal & ((1u << lane) - 1u))] = (u32)(hi - 1 - i); // = tid, kept for clarity
+        if (cand) {
+            const u32 slot = off + __popc(bal & ((1u << lane) - 1u));
+            s_rec[slot] = r_mine;
+            s_ab[slot] = ((u32)a_mine << 16) | (u32)b_mine;
+        }
         __syncthreads();
         if (tid == 0) {
             u32 m = s_merges;
             for (u32 c = 0; c < tot && m < (u32)(n - 1); ++c) {
-                const u64 r = rec[hi - 1 - s_list[c]];
-                int a, b;
-                edge_vertices((u32)r, &a, &b);
-                u32 ra = find_root(parent, a), rb = find_root(parent, b);
+                const u64 r = s_rec[c];
+                const u32 ab = s_ab[c];
+                u32 ra = find_root(parent, ab >> 16), rb = find_root(parent, ab & 0xffffu);
                 if (ra == rb) continue;
                 // a component is born with its largest vertex (vertices enter in decreasing index,
                 // PAPER.md:79); the younger component, the one with the smaller largest vertex, dies

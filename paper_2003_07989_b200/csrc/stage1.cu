@@ -80,32 +80,37 @@ __device__ __forceinline__ int summary_scan(const KT* __restrict__ Kf, const KT*
     int res = -1;
     const KT* __restrict__ sx = Sf + (size_t)xq * spitch;
     const KT* __restrict__ s1 = Sf + (size_t)v1q * spitch;
+    const KT* __restrict__ rx = Kf + xs + (31 - lane); // vertex 32 blk + 31 - lane of the two rows: r[32 blk]
+    const KT* __restrict__ r1 = Kf + v1s + (31 - lane);
+    const int nl = n - (31 - lane);                      // 32 blk < nl: the vertex exists
     for (int bt = base >> 5; bt >= 0 && res < 0; bt -= 32) {
         const int b = bt - lane;
         u32 s = 0u;
         if (b >= 0) s = min((u32)__ldg(sx + b), (u32)__ldg(s1 + b));
         u32 cand = __ballot_sync(RIPS_FULL_MASK, s >= ks);
         while (cand && res < 0) {
-            int blk[4];
-            u32 mm[4];
+            int b32[4]; // 32 x block, or past the end of the rows for an absent one
+            u32 mm[4], bb[4];
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
-                blk[g] = -1;
+                b32[g] = 0x7fffffe0;
                 if (cand) {
-                    blk[g] = bt - (__ffs(cand) - 1);
+                    b32[g] = (bt - (__ffs(cand) - 1)) << 5;
                     cand &= cand - 1;
                 }
             }
 #pragma unroll
             for (int g = 0; g < 4; ++g) {
-                const int vv = blk[g] * 32 + 31 - lane;
                 mm[g] = 0u;
-                if (blk[g] >= 0 && vv < n) mm[g] = min(min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]), extra(vv));
+                if (b32[g] < nl) mm[g] = min(min((u32)rx[b32[g]], (u32)r1[b32[g]]), extra(b32[g] + 31 - lane));
             }
 #pragma unroll
-            for (int g = 0; g < 4; ++g) {
-                const u32 bb = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
-                if (bb && res < 0) res = blk[g] * 32 + 31 - (__ffs(bb) - 1);
+            for (int g = 0; g < 4; ++g) bb[g] = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
+            if (bb[0] | bb[1] | bb[2] | bb[3]) { // the first block of the round that holds one, its highest vertex
+                const int g0 = bb[0] ? 0 : bb[1] ? 1 : bb[2] ? 2 : 3;
+                const u32 bg = bb[0] ? bb[0] : bb[1] ? bb[1] : bb[2] ? bb[2] : bb[3];
+                const int bg32 = g0 == 0 ? b32[0] : g0 == 1 ? b32[1] : g0 == 2 ? b32[2] : b32[3];
+                res = bg32 + 31 - (__ffs(bg) - 1);
             }
         }
     }
