@@ -199,7 +199,6 @@ struct rips_ctx {
     cudaEvent_t ev_join = nullptr, ev_join3 = nullptr, ev_fused = nullptr;
     int kmax = 0; // binomial table holds C(v,k), k <= kmax
     std::vector<u64> h_binom;
-    std::vector<float> h_values;
     float* d_dist = nullptr;
     u64* d_edges = nullptr; // sorted edge records (value descending, cidx ascending)
     u32* d_K = nullptr;
@@ -1119,6 +1118,10 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         CU(cudaMemcpyAsync(c->h_counters, c->d_counters, 24, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         c->edge_share = E ? (double)(E - (i64)c->h_counters[2]) / (double)E : 1.0;
+        // keys are ranks in descending value order: thr_key = number of distinct values above the threshold, and
+        // prep_edges_kernel made ONE value (+inf) of all of them -- so the table of values stays on the device
+        // (800 MB at n = 20000, which the host never needs)
+        c->thr_key = c->h_counters[2] != 0 ? 1u : 0u;
         release(c, c->b_init_tmp);
         release(c, c->b_init_status);
         if ((int)c->h_counters[1] != 0) {
@@ -1127,8 +1130,6 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         }
         c->n_distinct = (u32)c->h_counters[0];
         c->kf_u16 = c->n_distinct <= 65535u; // entries are key+1 <= n_distinct
-        c->h_values.resize(c->n_distinct);
-        CU(cudaMemcpy(c->h_values.data(), c->d_values, (size_t)c->n_distinct * 4, cudaMemcpyDeviceToHost));
     }
     {
         // row pitch: an odd number of 32-bit words, so the rows of consecutive vertices start in
@@ -1152,14 +1153,6 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         }
         c->vbits = bits_for((u64)(n - 1));
     }
-    // keys are ranks in descending value order: thr_key = number of distinct values above the threshold
-    u32 lo = 0, hi = c->n_distinct;
-    while (lo < hi) {
-        u32 mid = (lo + hi) / 2;
-        if (c->h_values[mid] > c->threshold) lo = mid + 1;
-        else hi = mid;
-    }
-    c->thr_key = lo;
     c->key_bits = bits_for(c->n_distinct); // the value n_distinct itself is the key of the column sentinel
     return RIPS_OK;
 }
