@@ -857,7 +857,13 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
         // slot mode: the leaner kernel, if its tables fit (C(., M+1) and one row of U2 per warp)
         const size_t u2rows = M > 2 ? (size_t)S1_WARPS * ((p.n + 7) & ~7) * sizeof(KT) : 0;
         const size_t tables = (size_t)p.n * 8 + u2rows;
-        if (p.Sf && u2rows <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, true>, p, u2rows, st);
+#ifdef RIPS_STRESS
+        const size_t u2_limit = 8 * 1024; // beyond ~130 points the triangles and tetrahedra go to the general kernel (its slot mode with block maxima)
+#else
+        const size_t u2_limit = 160 * 1024;
+#endif
+        if (p.Sf && u2rows <= u2_limit) return launch_persistent(enumerate_slot_kernel<M, KT, false, true>, p, u2rows, st);
+        if (p.Sf && u2rows > u2_limit && u2_limit < 160 * 1024) return launch_persistent(enumerate_apparent_kernel<M, KT, false>, p, 0, st);
         if (kf_fits && kf_bytes + tables <= 190 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, true, false>, p, kf_bytes + tables, st);
         if (tables <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, false>, p, tables, st);
     }

@@ -135,6 +135,11 @@ def test_stress_build(R):
             check_against_oracle(R, w.dist, w.n, 2, inf, "stress reduction")
             w = inputs.config(2, 40)
             check_against_oracle(R, w.dist, w.n, 3, inf, "stress slot")
+        # the stress build sends the triangles of more than ~130 points to the general kernel in slot mode, and builds
+        # the block maxima for every input: that kernel's scan guided by them (in the product build: n >= 2048 with
+        # tables that do not fit shared memory)
+        w = inputs.config(2, 140)
+        check_against_oracle(R, w.dist, w.n, 2, inf, "stress general kernel, slot mode, block maxima")
     finally:
         R.use_library(None)
 
