@@ -80,6 +80,13 @@ __global__ void __launch_bounds__(HIST_THREADS) sort_histogram_kernel(const u64*
 // look-back at once, scan over the bins; (4) records placed in tile-sorted order in shared memory;
 // (5) decoupled look-back per bin; (6) scatter, consecutive threads writing consecutive slots.
 // ----------------------------------------------------------------------------------------------
+// BALLOT: how the lanes that share a digit find each other.  One MATCH per record costs ~2 cycles per DISTINCT digit in
+// the warp; one ballot per digit bit costs the same whatever the digits.  MATCH wins while a warp's 32 records share a
+// few digits (keys of neighbouring simplices of dimension >= 2, cofacet vertices: 0.27 / 0.24 against 0.30 / 0.31 ms
+// per pass at cfg 2), ballots win when they are all different (keys of the edges: 1.15 against 1.50 ms per pass on a
+// random matrix of 20000 points).  Two instantiations rather than a branch: with both in one kernel the MATCH path
+// lost 9 % (measured).  The caller says which passes are of the second kind (sort_u64's ballot_passes).
+template <bool BALLOT>
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS)
 onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, const u64* __restrict__ n_dev, int shift, int bits,
                      const u64* __restrict__ hist_raw, u64* status, u32* ticket, int pf_dist)
@@ -164,9 +171,16 @@ onesweep_pass_kernel(const u64* __restrict__ in, u64* __restrict__ out, i64 n, c
 #pragma unroll
         for (int i = h; i < h + SORT_RANK_BATCH; ++i) {
             const u32 d = (u32)(key[i] >> shift) & mask;
-            // one MATCH per record (~2 cycles per distinct digit in the warp); one ballot per digit bit was
-            // measured slower at every pass of this workload
-            rank[i] = __match_any_sync(RIPS_FULL_MASK, d);
+            if (BALLOT) {
+                u32 peers = RIPS_FULL_MASK;
+                for (int b = 0; b < bits; ++b) {
+                    const bool one = (d >> b) & 1u;
+                    const u32 v = __ballot_sync(RIPS_FULL_MASK, one);
+                    peers &= one ? v : ~v;
+                }
+                rank[i] = peers;
+            } else
+                rank[i] = __match_any_sync(RIPS_FULL_MASK, d);
         }
         u32 old[SORT_RANK_BATCH];
 #pragma unroll
@@ -380,7 +394,7 @@ cudaError_t sort_prepare_fused(void* scratch, i64 n, const SortPlan& plan, cudaS
 }
 
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream, u64** result,
-                     SortTimes* times, i64* launches, bool hist_ready, bool skewed_digits, const u64* n_dev)
+                     SortTimes* times, i64* launches, bool hist_ready, u32 ballot_passes, const u64* n_dev)
 {
     *result = a;
     int sms = 148;
@@ -400,14 +414,15 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
         return cudaSuccess;
     }
     {   // per call (cheap) rather than once per process: the attribute is per device
-        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
+        cudaError_t e = cudaFuncSetAttribute(onesweep_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(onesweep_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pass_smem_bytes(8));
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(sort_histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  RIPS_SORT_MAX_PASSES * RIPS_SORT_MAX_BINS * 4);
         if (e != cudaSuccess) return e;
     }
     const int pf_dist = sms; // tiles ahead of the L2 prefetch: one wave (swept 0 .. 12 waves in round 1)
-    (void)skewed_digits;
     ScratchLayout L = scratch_layout(n, plan);
     unsigned char* sc = (unsigned char*)scratch;
     u64* hist = (u64*)(sc + L.hist_off);
@@ -433,8 +448,12 @@ cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch,
     u64* src = a;
     u64* dst = b;
     for (int p = 0; p < plan.npasses; ++p) {
-        onesweep_pass_kernel<<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
-            src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, (u64*)(sc + L.status_off[p]), ticket + p, pf_dist);
+        if ((ballot_passes >> p) & 1u)
+            onesweep_pass_kernel<true><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
+                src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, (u64*)(sc + L.status_off[p]), ticket + p, pf_dist);
+        else
+            onesweep_pass_kernel<false><<<(unsigned)tiles, SORT_THREADS, pass_smem_bytes(plan.bits[p]), stream>>>(
+                src, dst, n, n_dev, plan.shift[p], plan.bits[p], hist + (size_t)p * RIPS_SORT_MAX_BINS, (u64*)(sc + L.status_off[p]), ticket + p, pf_dist);
         if (launches) *launches += 1;
         u64* t = src; src = dst; dst = t;
     }

@@ -32,12 +32,13 @@ struct SortTimes {
 // hist_ready: the caller zeroed the scratch head with sort_prepare_fused and a producer kernel has
 // already accumulated the raw digit counts of every pass into sort_hist_ptr(scratch)[pass][256]
 // (FusedHist in kernels.cuh); the sort then skips its own histogram read of the records.
-// skewed_digits: a warp's 32 records mostly share a few digits (ranking by MATCH instead of ballots).
+// ballot_passes: bit p set = the 32 records of a warp mostly differ in the digit of pass p (keys of edges, mantissa bits):
+// that pass ranks by ballots instead of MATCH (radix_sort.cu, onesweep_pass_kernel).  Any value gives the same result.
 // n_dev (optional): the number of records lives on the device (u64); n is then its upper bound (launch size, scratch size)
 // and the kernels sort min(*n_dev, n) records.  Whatever the count, the sorted data ends in *result.
 cudaError_t sort_u64(u64* a, u64* b, i64 n, const SortPlan& plan, void* scratch, cudaStream_t stream,
                      u64** result, SortTimes* times, i64* launches, bool hist_ready = false,
-                     bool skewed_digits = false, const u64* n_dev = nullptr);
+                     u32 ballot_passes = 0, const u64* n_dev = nullptr);
 // (clears the whole scratch of a sort of n records: histograms, tickets, the status words of every pass)
 cudaError_t sort_prepare_fused(void* scratch, i64 n, const SortPlan& plan, cudaStream_t stream);
 

@@ -588,7 +588,8 @@ int run_stage1_sparse(rips_ctx* c, int d)
         st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
         s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, total, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, false));
+        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, total, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, false,
+                    s.M == 2 ? 0xffu : 0u)); // the keys of edges differ inside a warp, those of neighbouring triangles mostly do not
         s.cols = res;
         ev_record(c, s, EV_S1_END);
     }
@@ -815,7 +816,8 @@ int run_stage1(rips_ctx* c, int d)
         st.ev[0] = s.ev[EV_S1_SORTBEG]; st.ev[1] = s.ev[EV_S1_HIST]; st.ev[2] = s.ev[EV_S1_SORT];
         s.ev_rec[EV_S1_SORTBEG] = s.ev_rec[EV_S1_HIST] = s.ev_rec[EV_S1_SORT] = true;
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, (i64)cap, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused));
+        CU(sort_u64((u64*)s.colsA.p, (u64*)s.colsB.p, (i64)cap, plan, c->sort_scratch.p, c->stream, &res, &st, &c->launches, fused,
+                    s.M == 2 ? 0xffu : 0u)); // the keys of edges differ inside a warp, those of neighbouring triangles mostly do not
         s.cols = res;
         ev_record(c, s, EV_S1_END);
     }
@@ -865,7 +867,7 @@ int run_stage2(rips_ctx* c, int d)
         s.ev_rec[EV_S2_SORTBEG] = s.ev_rec[EV_S2_HIST] = s.ev_rec[EV_S2_SORT] = true;
         u64* res = nullptr;
         CU(sort_u64((u64*)s.pairsA.p, (u64*)s.pairsB.p, s.slots, s.pair_plan, s.pair_scratch.p, c->stream, &res, &st,
-                    &c->launches, s.pair_fused, true));
+                    &c->launches, s.pair_fused, 0u)); // cofacet vertices: a few values per warp
         s.reg = res;
     }
     // ---- a8: the two small out-of-order lists: irregular pairs by cidx(t), non-apparent columns by
@@ -875,13 +877,13 @@ int run_stage2(rips_ctx* c, int d)
         RC(ensure(c, s.irrB, (size_t)s.irr_cap * 8));
         RC(ensure(c, c->sort_scratch2, sort_scratch_bytes((i64)s.irr_cap, pi)));
         u64* res = nullptr;
-        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, irr_n, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches, false, false,
+        CU(sort_u64((u64*)s.irrA.p, (u64*)s.irrB.p, irr_n, pi, c->sort_scratch2.p, st2, &res, nullptr, &c->launches, false, 0u,
                     d_cnt + S1C_IRREGULAR));
         s.irr = res;
         SortPlan pn = sort_make_plan(0, s.lowbits + c->key_bits);
         RC(ensure(c, s.nonB, (size_t)s.non_cap * 8));
         RC(ensure(c, c->sort_scratch3, sort_scratch_bytes((i64)s.non_cap, pn)));
-        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, non_n, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches, false, false,
+        CU(sort_u64((u64*)s.nonA.p, (u64*)s.nonB.p, non_n, pn, c->sort_scratch3.p, st3, &res, nullptr, &c->launches, false, 0u,
                     d_cnt + S1C_NONAPP));
         if (st3 != st2) { // join the third stream into the second
             CU(cudaEventRecord(c->ev_join3, st3));
@@ -1109,7 +1111,8 @@ int init_device_tables(rips_ctx* c, const float* dist_lower)
         SortPlan plan = sort_make_plan(32, 64);
         RC(ensure(c, c->sort_scratch, sort_scratch_bytes(E, plan)));
         u64* res = nullptr;
-        CU(sort_u64(c->d_edges, (u64*)c->b_init_tmp.p, E, plan, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches));
+        CU(sort_u64(c->d_edges, (u64*)c->b_init_tmp.p, E, plan, c->sort_scratch.p, c->stream, &res, nullptr, &c->launches, false,
+                    0x7u)); // fp32 bits: the mantissa bytes differ inside a warp, the exponent byte does not
         if (res != c->d_edges) { std::swap(c->b_edges, c->b_init_tmp); c->d_edges = (u64*)c->b_edges.p; }
         RC(ensure(c, c->b_init_status, (size_t)rank_edges_tiles(E) * 8));
         CU(cudaMemsetAsync(c->b_init_status.p, 0, (size_t)rank_edges_tiles(E) * 8, c->stream));
