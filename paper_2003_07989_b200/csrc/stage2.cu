@@ -29,6 +29,16 @@ __device__ __forceinline__ u64 pair_s_of(const BinomTable& bt, int n, u64 rec)
     return s;
 }
 
+__device__ __forceinline__ i64 lower_bound_field_in(const u64* __restrict__ a, i64 lo, i64 hi, int shift, u64 mask, u64 x)
+{
+    while (lo < hi) {
+        i64 mid = lo + ((hi - lo) >> 1);
+        if (((__ldg(a + mid) >> shift) & mask) < x) lo = mid + 1;
+        else hi = mid;
+    }
+    return lo;
+}
+
 __device__ __forceinline__ i64 lower_bound_field(const u64* __restrict__ a, i64 n, int shift, u64 mask, u64 x)
 {
     i64 lo = 0, hi = n;
@@ -57,25 +67,41 @@ __global__ void unpack_columns_kernel(const u64* __restrict__ cols, i64 len, int
 
 // Apparent pairs ascending by t: merge of the regular and the irregular layer.  Rows are distinct,
 // so element i of one layer lands at i + #{rows of the other layer below it}.
+constexpr int MA_THREADS = 256, MA_ITEMS = 8; // rows per block: MA_THREADS * MA_ITEMS
 template <int M>
-__global__ void merge_apparent_kernel(PairLayers L, BinomTable bt, int n, u64* __restrict__ t, u64* __restrict__ s)
+__global__ void __launch_bounds__(MA_THREADS) merge_apparent_kernel(PairLayers L, BinomTable bt, int n, u64* __restrict__ t, u64* __restrict__ s)
 {
-    i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
     const u64 tmask = (L.tbits >= 64) ? ~0ull : ((1ull << L.tbits) - 1ull);
-    if (i < L.n_reg) {
-        const u64 r = __ldg(L.reg + i);
-        const u64 tt = r & tmask;
-        const int v = (int)(r >> L.tbits);
-        const i64 pos = i + lower_bound_field(L.irr, L.n_irr, RIPS_PAIR_POS_BITS, ~0ull, tt);
-        t[pos] = tt;
-        s[pos] = tt - bt(v, M + 1);
-    } else if (i < L.n_reg + L.n_irr) {
-        const i64 k = i - L.n_reg;
-        const u64 r = __ldg(L.irr + k);
-        const u64 tt = r >> RIPS_PAIR_POS_BITS;
-        const i64 pos = k + lower_bound_field(L.reg, L.n_reg, 0, tmask, tt);
-        t[pos] = tt;
-        s[pos] = pair_s_of<M>(bt, n, r);
+    const i64 b0 = (i64)blockIdx.x * (MA_THREADS * MA_ITEMS);
+    // the regular rows of a block are ascending, so their places in the irregular layer lie between those of the
+    // block's first and last row: two searches through the whole layer per block of 2048 rows (their ~20 dependent
+    // loads each were the kernel's run time when every row, and then every 256 rows, made them), the others through
+    // that window
+    __shared__ i64 s_win[2];
+    if (b0 < L.n_reg && (threadIdx.x == 0 || threadIdx.x == 32)) {
+        const i64 b1 = (b0 + MA_THREADS * MA_ITEMS - 1 < L.n_reg) ? b0 + MA_THREADS * MA_ITEMS - 1 : L.n_reg - 1;
+        const u64 tb = __ldg(L.reg + (threadIdx.x == 0 ? b0 : b1)) & tmask;
+        s_win[threadIdx.x == 0 ? 0 : 1] = lower_bound_field(L.irr, L.n_irr, RIPS_PAIR_POS_BITS, ~0ull, tb);
+    }
+    __syncthreads();
+#pragma unroll 4
+    for (int it = 0; it < MA_ITEMS; ++it) {
+        const i64 i = b0 + (i64)it * MA_THREADS + threadIdx.x;
+        if (i < L.n_reg) {
+            const u64 r = __ldg(L.reg + i);
+            const u64 tt = r & tmask;
+            const int v = (int)(r >> L.tbits);
+            const i64 pos = i + lower_bound_field_in(L.irr, s_win[0], s_win[1], RIPS_PAIR_POS_BITS, ~0ull, tt);
+            t[pos] = tt;
+            s[pos] = tt - bt(v, M + 1);
+        } else if (i < L.n_reg + L.n_irr) {
+            const i64 k = i - L.n_reg;
+            const u64 r = __ldg(L.irr + k);
+            const u64 tt = r >> RIPS_PAIR_POS_BITS;
+            const i64 pos = k + lower_bound_field(L.reg, L.n_reg, 0, tmask, tt);
+            t[pos] = tt;
+            s[pos] = pair_s_of<M>(bt, n, r);
+        }
     }
 }
 
@@ -149,8 +175,8 @@ cudaError_t launch_merge_apparent(int M, const PairLayers& L, BinomTable bt, int
 {
     const i64 tot = L.n_reg + L.n_irr;
     if (tot == 0) return cudaSuccess;
-    unsigned g = (unsigned)((tot + 255) / 256);
-    RIPS_DISPATCH_M(M, (merge_apparent_kernel<MM><<<g, 256, 0, st>>>(L, bt, n, t, s)));
+    unsigned g = (unsigned)((tot + MA_THREADS * MA_ITEMS - 1) / (MA_THREADS * MA_ITEMS));
+    RIPS_DISPATCH_M(M, (merge_apparent_kernel<MM><<<g, MA_THREADS, 0, st>>>(L, bt, n, t, s)));
     return cudaGetLastError();
 }
 
