@@ -105,22 +105,34 @@ __global__ void __launch_bounds__(MA_THREADS) merge_apparent_kernel(PairLayers L
     }
 }
 
-// merge of two (t, s) arrays with distinct t, both ascending
-__global__ void merge_ts_kernel(const u64* __restrict__ t1, const u64* __restrict__ s1, i64 n1, const u64* __restrict__ t2,
-                                const u64* __restrict__ s2, i64 n2, u64* __restrict__ t, u64* __restrict__ s)
+// merge of two (t, s) arrays with distinct t, both ascending (the first one the long one: the same windowed search
+// as merge_apparent_kernel)
+__global__ void __launch_bounds__(MA_THREADS) merge_ts_kernel(const u64* __restrict__ t1, const u64* __restrict__ s1, i64 n1,
+                                                            const u64* __restrict__ t2, const u64* __restrict__ s2, i64 n2,
+                                                            u64* __restrict__ t, u64* __restrict__ s)
 {
-    i64 i = (i64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n1) {
-        const u64 tt = __ldg(t1 + i);
-        const i64 pos = i + lower_bound_field(t2, n2, 0, ~0ull, tt);
-        t[pos] = tt;
-        s[pos] = __ldg(s1 + i);
-    } else if (i < n1 + n2) {
-        const i64 k = i - n1;
-        const u64 tt = __ldg(t2 + k);
-        const i64 pos = k + lower_bound_field(t1, n1, 0, ~0ull, tt);
-        t[pos] = tt;
-        s[pos] = __ldg(s2 + k);
+    const i64 b0 = (i64)blockIdx.x * (MA_THREADS * MA_ITEMS);
+    __shared__ i64 s_win[2];
+    if (b0 < n1 && (threadIdx.x == 0 || threadIdx.x == 32)) {
+        const i64 b1 = (b0 + MA_THREADS * MA_ITEMS - 1 < n1) ? b0 + MA_THREADS * MA_ITEMS - 1 : n1 - 1;
+        s_win[threadIdx.x == 0 ? 0 : 1] = lower_bound_field(t2, n2, 0, ~0ull, __ldg(t1 + (threadIdx.x == 0 ? b0 : b1)));
+    }
+    __syncthreads();
+#pragma unroll 4
+    for (int it = 0; it < MA_ITEMS; ++it) {
+        const i64 i = b0 + (i64)it * MA_THREADS + threadIdx.x;
+        if (i < n1) {
+            const u64 tt = __ldg(t1 + i);
+            const i64 pos = i + lower_bound_field_in(t2, s_win[0], s_win[1], 0, ~0ull, tt);
+            t[pos] = tt;
+            s[pos] = __ldg(s1 + i);
+        } else if (i < n1 + n2) {
+            const i64 k = i - n1;
+            const u64 tt = __ldg(t2 + k);
+            const i64 pos = k + lower_bound_field(t1, n1, 0, ~0ull, tt);
+            t[pos] = tt;
+            s[pos] = __ldg(s2 + k);
+        }
     }
 }
 
@@ -184,8 +196,8 @@ cudaError_t launch_merge_ts(const u64* t1, const u64* s1, i64 n1, const u64* t2,
                             cudaStream_t st)
 {
     if (n1 + n2 == 0) return cudaSuccess;
-    unsigned g = (unsigned)((n1 + n2 + 255) / 256);
-    merge_ts_kernel<<<g, 256, 0, st>>>(t1, s1, n1, t2, s2, n2, t, s);
+    unsigned g = (unsigned)((n1 + n2 + MA_THREADS * MA_ITEMS - 1) / (MA_THREADS * MA_ITEMS));
+    merge_ts_kernel<<<g, MA_THREADS, 0, st>>>(t1, s1, n1, t2, s2, n2, t, s);
     return cudaGetLastError();
 }
 
