@@ -22,17 +22,20 @@ __device__ __forceinline__ void edge_vertices(u32 e, int* a, int* b)
     *b = (int)(e - (u32)((u64)i * (u64)(i - 1) / 2));
 }
 
-__device__ __forceinline__ u32 find_root(volatile u32* parent, u32 x)
+typedef unsigned short u16; // vertex numbers: n <= 46340 (rips_init)
+
+__device__ __forceinline__ u32 find_root(volatile u16* parent, u32 x)
 {
     u32 r = x;
     while (parent[r] != r) r = parent[r];
     // compression: every write stores an ancestor, so concurrent readers always see a valid forest
-    while (parent[x] != r) { u32 nx = parent[x]; parent[x] = r; x = nx; }
+    while (parent[x] != r) { u32 nx = parent[x]; parent[x] = (u16)r; x = nx; }
     return r;
 }
 
-// SM: the union-find arrays (parent, largest vertex per root: 8 bytes per vertex) live in shared memory
-// (n <= 25000); else in the global scratch the caller passed.  The merges are serial, so their latency is
+// SM: the union-find arrays (parent, largest vertex per root: 16 bits each, 4 bytes per vertex) live in shared memory
+// (every n rips_init admits: 181 KB at n = 46340; as 32-bit words they left shared memory at n = 25000, and the kernel
+// with its forest in HBM took 59 ms at n = 40000 instead of 14); else in the global scratch the caller passed.  The merges are serial, so their latency is
 // the kernel's run time.
 template <bool SM>
 __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict__ rec, i64 E, int n, u32 thr_inv,
@@ -45,10 +48,10 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
     __shared__ u32 s_wcount[D0_THREADS / 32];
     __shared__ i64 s_start;
     __shared__ u32 s_merges;
-    volatile u32* parent = parent_maxv;
-    volatile u32* maxv = parent_maxv + n;
+    volatile u16* parent = reinterpret_cast<volatile u16*>(parent_maxv);
+    volatile u16* maxv = parent + n;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int i = tid; i < n; i += D0_THREADS) { parent[i] = i; maxv[i] = i; }
+    for (int i = tid; i < n; i += D0_THREADS) { parent[i] = (u16)i; maxv[i] = (u16)i; }
     if (tid == 0) {
         // first position whose value is <= threshold (records are value-descending = inverted bits ascending)
         i64 lo = 0, hi = E;
@@ -100,7 +103,7 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
                 u32 living = (dying == ra) ? rb : ra;
                 out.pair_ts[m] = ((u64)(u32)r << 16) | (u64)maxv[dying];
                 out.death[m] = __uint_as_float(~(u32)(r >> 32));
-                parent[dying] = living;
+                parent[dying] = (u16)living;
                 ++m;
             }
             s_merges = m;
@@ -116,8 +119,8 @@ __global__ void __launch_bounds__(D0_THREADS) dim0_kernel(const u64* __restrict_
 cudaError_t launch_dim0(const u64* rec_sorted, i64 E, int n, u32 thr_bits_inv, u32* parent_maxv, Dim0Out out,
                         cudaStream_t st)
 {
-    const size_t bytes = (size_t)n * 8;
-    if (bytes <= 200 * 1024) {
+    const size_t bytes = ((size_t)n * 4 + 15) & ~(size_t)15;
+    if (n <= 65535 && bytes <= 200 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(dim0_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         dim0_kernel<true><<<1, D0_THREADS, bytes, st>>>(rec_sorted, E, n, thr_bits_inv, parent_maxv, out);

@@ -177,6 +177,33 @@ def test_block_maxima_guide_the_scan_in_both_fused_kernels(R):
                 assert 0.39 * comb(w.n, 2) < st["n_columns"] + st["n_cleared"] < 0.41 * comb(w.n, 2)
 
 
+def test_dimension0_with_vertex_numbers_beyond_15_bits(R):
+    """33,000 points on a line at distinct integer positions (fp32-exact distances, many of them equal): dim0_kernel
+    keeps its forest as 16-bit vertex numbers in shared memory for every n rips_init admits.  The finite bars of
+    dimension 0 are the edges of a minimum spanning tree, whose multiset of weights is unique whatever the ties: the
+    gaps between neighbours on the line (a closed form, not the oracle: its dimension 0 needs minutes at this size).
+    The pivots must be edges of that weight, and every vertex but one must die exactly once."""
+    n = 33000
+    rng = np.random.default_rng(11)
+    pos = rng.choice(1 << 23, n, replace=False).astype(np.float32)
+    low = np.empty(n * (n - 1) // 2, dtype=np.float32)
+    for i in range(1, n):
+        low[i * (i - 1) // 2: i * (i + 1) // 2] = np.abs(pos[i] - pos[:i])
+    gaps = np.sort(np.diff(np.sort(pos)))
+    with R.Rips(low, n, 0) as g:
+        g.dim0()
+        bars = g.barcodes(0)
+        assert bars.shape[0] == n                                    # n - 1 finite bars and the essential one
+        fin = bars[np.isfinite(bars[:, 1])]
+        assert fin.shape[0] == n - 1 and np.all(fin[:, 0] == 0)
+        assert np.array_equal(np.sort(fin[:, 1]), gaps)
+        pt, ps = g.pivots(0)                                         # (edge, vertex that dies with it)
+        e = pt.cpu().numpy().astype(np.int64)
+        v = ps.cpu().numpy().astype(np.int64)
+        assert np.array_equal(np.sort(low[e]), gaps)
+        assert np.unique(v).size == n - 1 and v.min() >= 0 and v.max() < n
+
+
 def test_config4_through_both_paths(R):
     """Config 4 (1000 points, threshold 0.15: 1.2 % of the edges) at full size through the sparse path (what
     RIPS_MODE_AUTO picks for it) and through the dense path: every array of every dimension against the oracle."""
