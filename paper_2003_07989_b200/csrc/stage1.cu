@@ -30,6 +30,8 @@ namespace {
 
 constexpr int S1_THREADS = 1024;
 constexpr int S1_WARPS = S1_THREADS / 32;
+constexpr int S1_QCAP = 64;     // slot kernel: entries of a warp's queue of open cofacet scans (31 waiting + 32 new at most)
+constexpr int S1_QVISITS = 12;  // cofacet vertices every drained candidate tests on its own before the warp takes its scan over
 constexpr int S1_CHUNK = 1024;         // most candidates per warp chunk (unit of work and of the look-back chain)
 constexpr int S1_MAX_FUSED = 3;        // digits of the filtration sort histogrammed on the way out
 constexpr int S1_MAX_FUSED_P = 2;      // digits of the pair partition
@@ -533,6 +535,12 @@ __global__ void __launch_bounds__(S1_THREADS, SUM ? 2 : 0) enumerate_slot_kernel
         off_b += (size_t)n * 8;
     }
     KT* const u2 = reinterpret_cast<KT*>(smem1 + off_b) + (size_t)warp * ((n + 7) & ~7);
+    // (!SUM) the warp's queue of candidates whose cofacet scan is still open after four vertices: S1_QCAP entries of
+    // (cidx, key, v1, v0), behind the U2 rows
+    const size_t q_off = (off_b + ((M > 2) ? (size_t)S1_WARPS * ((n + 7) & ~7) * sizeof(KT) : 0) + 15) & ~(size_t)15;
+    uint4* const q = reinterpret_cast<uint4*>(smem1 + q_off) + (size_t)warp * S1_QCAP;
+    int qcnt = 0;
+    const u32 lt_mask_q = (1u << lane) - 1u;
     for (int i = tid; i < S1_MAX_FUSED * 256; i += S1_THREADS) (&s_hist_cols[0][0])[i] = 0;
     for (int i = tid; i < S1_MAX_FUSED_P * 256; i += S1_THREADS) (&s_hist_pairs[0][0])[i] = 0;
     __syncthreads();
@@ -593,6 +601,111 @@ __global__ void __launch_bounds__(S1_THREADS, SUM ? 2 : 0) enumerate_slot_kernel
             }
             const int vtop_slab = (M > 2) ? v[M - 1] : 0;
 
+            // ---- what follows the cofacet scan of a candidate: the pair slot, the pair histogram, and for a cofacet vertex
+            // below the top of s (whole rows of lanes: the columns holding the top vertices) or no cofacet of equal diameter
+            // the facet test and the two small lists.  Called by the whole warp: in the walk for the lanes whose scan
+            // ended within four vertices (and the dropped candidates), in drain() for the others.
+            auto finish = [&](const bool act, const bool keep_, const u64 ci_, const u32 key1_, const int lv1_, const int lx_, const int fv_) {
+                const bool found = fv_ >= 0;
+                const int vtop = (M > 2) ? vtop_slab : lv1_;
+                const bool regular = act && found && fv_ > vtop;
+                const u32 fvv = regular ? (u32)fv_ : (u32)n;
+                u64 prec = psentinel;
+                if (regular) {
+                    prec = SUM ? ci_ + ((u64)(u32)fv_ << p.tbits) + p.bt(fv_, M + 1) : ci_ + sprec[fv_];
+                    ++n_reg;
+                }
+                if (__any_sync(RIPS_FULL_MASK, act && keep_ && !regular)) {
+                    bool is_irr = false, is_non = act && keep_ && !found;
+                    u64 irr_rec = 0;
+                    if (act && keep_ && found && !regular) {
+                        int sv[M];
+                        sv[0] = lx_;
+                        sv[1] = lv1_;
+#pragma unroll
+                        for (int j = 2; j < M; ++j) sv[j] = v[j];
+                        int fseg = 0;
+#pragma unroll
+                        for (int j = 0; j < M; ++j) fseg += (sv[j] < fv_) ? 1 : 0;
+                        if (s_is_youngest_facet<M, KT>(Kf, pitch, sv, key1_, fv_, fseg)) {
+                            irr_rec = (cofacet_index<M>(p.bt, sv, fv_, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
+                            is_irr = true;
+                        } else
+                            is_non = true;
+                    }
+                    const u32 lt_mask = (1u << lane) - 1u;
+                    const u32 b_irr = __ballot_sync(RIPS_FULL_MASK, is_irr);
+                    if (b_irr) {
+                        u64 base = 0;
+                        if (lane == __ffs(b_irr) - 1)
+                            base = atomicAdd((unsigned long long*)(p.counters + S1C_IRREGULAR), (unsigned long long)__popc(b_irr));
+                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_irr) - 1) + __popc(b_irr & lt_mask);
+                        if (is_irr && base < p.irr_cap) p.irr_out[base] = irr_rec;
+                    }
+                    const u32 b_non = __ballot_sync(RIPS_FULL_MASK, is_non);
+                    if (b_non) {
+                        u64 base = 0;
+                        if (lane == __ffs(b_non) - 1)
+                            base = atomicAdd((unsigned long long*)(p.counters + S1C_NONAPP), (unsigned long long)__popc(b_non));
+                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_non) - 1) + __popc(b_non & lt_mask);
+                        if (is_non && base < p.non_cap)
+                            p.non_out[base] = ((u64)(key1_ - 1u) << lowbits) | slab_low | (u64)((u32)lv1_ * vmul + (u32)lx_);
+                    }
+                }
+                if (act) __stcs(p.pairs_out + ci_, prec);
+#pragma unroll
+                for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
+                    if (r < npd) { // few distinct digits in a warp: aggregate
+                        const u32 dg = act ? ((fvv >> (8 * r)) & 0xffu) : 0xffffffffu;
+                        const u32 peers = __match_any_sync(RIPS_FULL_MASK, dg);
+                        if (act && lane == __ffs(peers) - 1) atomicAdd(&s_hist_pairs[r][dg], (u32)__popc(peers));
+                    }
+                }
+            };
+            // ---- (!SUM) the last m entries of the warp's queue, one per lane: S1_QVISITS more cofacet vertices for every lane
+            // at once, branch-free (three in four end there), the rest by the whole warp, 32 vertices per step, then finish()
+            auto drain = [&](const int m) {
+                __syncwarp();
+                const bool act = lane < m;
+                const uint4 e = q[qcnt - m + (act ? lane : 0)];
+                qcnt -= m;
+                __syncwarp();
+                const u64 ci_ = ((u64)e.y << 32) | (u64)e.x;
+                const u32 key1_ = e.z;
+                const int lv1_ = (int)(e.w >> 16), lx_ = (int)(e.w & 0xffffu);
+                const int r1o_ = lv1_ * pitch, xo_ = lx_ * pitch;
+                const int kend = n < 4 + S1_QVISITS ? n : 4 + S1_QVISITS;
+                int fv_ = -1;
+#pragma unroll
+                for (int k = 4 + S1_QVISITS - 1; k >= 4; --k) {
+                    if (k < kend) {
+                        const u32 uu = (M > 2) ? (u32)u2[n - 1 - k] : 0xffffffffu;
+                        if (min(min(uu, (u32)Kf[r1o_ + n - 1 - k]), (u32)Kf[xo_ + n - 1 - k]) >= key1_) fv_ = n - 1 - k;
+                    }
+                }
+                u32 open = __ballot_sync(RIPS_FULL_MASK, act && fv_ < 0);
+                while (open) {
+                    const int src = __ffs(open) - 1;
+                    open &= open - 1;
+                    const int xs = __shfl_sync(RIPS_FULL_MASK, xo_, src);
+                    const int v1s = __shfl_sync(RIPS_FULL_MASK, r1o_, src);
+                    const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1_, src);
+                    int res = -1;
+                    for (int base = n - 1 - kend; base >= 0 && res < 0; base -= 32) {
+                        const int vv = base - lane;
+                        u32 m0 = 0u;
+                        if (vv >= 0) {
+                            m0 = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                            if (M > 2) m0 = min(m0, (u32)u2[vv]);
+                        }
+                        const u32 bb = __ballot_sync(RIPS_FULL_MASK, m0 >= ks); // (ks >= 1: an absent vertex never passes)
+                        if (bb) res = base - (__ffs(bb) - 1);
+                    }
+                    if (lane == src) fv_ = res;
+                }
+                finish(act, true, ci_, key1_, lv1_, lx_, fv_);
+            };
+
             // ---- the lanes walk the segment's pairs (v1, x) in index order, 32 at a time
             int lv1, lx;
             {
@@ -637,138 +750,96 @@ __global__ void __launch_bounds__(S1_THREADS, SUM ? 2 : 0) enumerate_slot_kernel
                     fv = h0 ? n - 1 : h1 ? n - 2 : h2 ? n - 3 : h3 ? n - 4 : -1;
                     if (!keep) fv = -1;
                 }
-                u32 open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
-                if (open && n > 4) { // four more for the lanes still open
-                    const int kend = n < 8 ? n : 8;
-                    if (keep && fv < 0) {
-                        for (int k = 4; k < kend; ++k) {
-                            const u32 uu = (M > 2) ? (u32)u2[n - 1 - k] : 0xffffffffu;
-                            if (min(min(uu, (u32)Kf[r1o + n - 1 - k]), (u32)Kf[xo + n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
-                        }
+                bool defer = false;
+                if (!SUM && n > 4) {
+                    // the lanes still open (one in ten) wait in the warp's queue and are finished 32 at a time (drain)
+                    defer = keep && fv < 0;
+                    const u32 db = __ballot_sync(RIPS_FULL_MASK, defer);
+                    if (db) {
+                        if (defer) q[qcnt + __popc(db & lt_mask_q)] = make_uint4((u32)ci, (u32)(ci >> 32), key1, ((u32)lv1 << 16) | (u32)lx);
+                        qcnt += __popc(db);
                     }
-                    open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
-                    // the rest by the whole warp, one open lane after the other, 32 cofacet vertices per step
-                    while (open) {
-                        const int src = __ffs(open) - 1;
-                        open &= open - 1;
-                        const int xs = __shfl_sync(RIPS_FULL_MASK, xo, src);
-                        const int v1s = __shfl_sync(RIPS_FULL_MASK, r1o, src);
-                        const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
-                        // (four groups of 32 vertices per round: the loads of a round are independent, so a column
-                        // without any cofacet of equal diameter -- a scan of all n vertices -- waits for HBM n/128
-                        // times, not n/32 times; that scan is what binds the kernel when n is in the thousands)
-                        int res = -1;
-                        int base = n - 1 - kend;
-                        if (base >= 0) { // the next 32 vertices first: most open lanes end here
-                            const int vv = base - lane;
-                            u32 m0 = 0u;
-                            if (vv >= 0) {
-                                m0 = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
-                                if (M > 2) m0 = min(m0, (u32)u2[vv]);
+                } else {
+                    u32 open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
+                    if (open && n > 4) { // four more for the lanes still open
+                        const int kend = n < 8 ? n : 8;
+                        if (keep && fv < 0) {
+                            for (int k = 4; k < kend; ++k) {
+                                const u32 uu = (M > 2) ? (u32)u2[n - 1 - k] : 0xffffffffu;
+                                if (min(min(uu, (u32)Kf[r1o + n - 1 - k]), (u32)Kf[xo + n - 1 - k]) >= key1) { fv = n - 1 - k; break; }
                             }
-                            const u32 bb = __ballot_sync(RIPS_FULL_MASK, m0 >= ks); // (ks >= 1: an absent vertex never passes)
-                            if (bb) res = base - (__ffs(bb) - 1);
-                            base -= 32;
                         }
-                        if (SUM) { // (the block maxima of the two rows say which blocks of 32 vertices are worth reading)
-                            const int xq = __shfl_sync(RIPS_FULL_MASK, lx, src);
-                            const int v1q = __shfl_sync(RIPS_FULL_MASK, lv1, src);
-                            if (res < 0)
-                                res = summary_scan<KT>(Kf, reinterpret_cast<const KT*>(p.Sf), p.spitch, n, xs, v1s, xq, v1q, ks, base, lane,
-                                                       [&](const int w) { return (M > 2) ? (u32)u2[w] : 0xffffffffu; });
-                            base = -1;
-                        }
-                        for (; base >= 0 && res < 0; base -= 128) {
-                            u32 mm[4];
-#pragma unroll
-                            for (int g = 0; g < 4; ++g) {
-                                const int vv = base - 32 * g - lane;
-                                mm[g] = 0u;
+                        open = __ballot_sync(RIPS_FULL_MASK, keep && fv < 0);
+                        // the rest by the whole warp, one open lane after the other, 32 cofacet vertices per step
+                        while (open) {
+                            const int src = __ffs(open) - 1;
+                            open &= open - 1;
+                            const int xs = __shfl_sync(RIPS_FULL_MASK, xo, src);
+                            const int v1s = __shfl_sync(RIPS_FULL_MASK, r1o, src);
+                            const u32 ks = __shfl_sync(RIPS_FULL_MASK, key1, src);
+                            // (four groups of 32 vertices per round: the loads of a round are independent, so a column
+                            // without any cofacet of equal diameter -- a scan of all n vertices -- waits for HBM n/128
+                            // times, not n/32 times; that scan is what binds the kernel when n is in the thousands)
+                            int res = -1;
+                            int base = n - 1 - kend;
+                            if (base >= 0) { // the next 32 vertices first: most open lanes end here
+                                const int vv = base - lane;
+                                u32 m0 = 0u;
                                 if (vv >= 0) {
-                                    mm[g] = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
-                                    if (M > 2) mm[g] = min(mm[g], (u32)u2[vv]);
+                                    m0 = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                                    if (M > 2) m0 = min(m0, (u32)u2[vv]);
+                                }
+                                const u32 bb = __ballot_sync(RIPS_FULL_MASK, m0 >= ks); // (ks >= 1: an absent vertex never passes)
+                                if (bb) res = base - (__ffs(bb) - 1);
+                                base -= 32;
+                            }
+                            if (SUM) { // (the block maxima of the two rows say which blocks of 32 vertices are worth reading)
+                                const int xq = __shfl_sync(RIPS_FULL_MASK, lx, src);
+                                const int v1q = __shfl_sync(RIPS_FULL_MASK, lv1, src);
+                                if (res < 0)
+                                    res = summary_scan<KT>(Kf, reinterpret_cast<const KT*>(p.Sf), p.spitch, n, xs, v1s, xq, v1q, ks, base, lane,
+                                                           [&](const int w) { return (M > 2) ? (u32)u2[w] : 0xffffffffu; });
+                                base = -1;
+                            }
+                            for (; base >= 0 && res < 0; base -= 128) {
+                                u32 mm[4];
+#pragma unroll
+                                for (int g = 0; g < 4; ++g) {
+                                    const int vv = base - 32 * g - lane;
+                                    mm[g] = 0u;
+                                    if (vv >= 0) {
+                                        mm[g] = min((u32)Kf[xs + vv], (u32)Kf[v1s + vv]);
+                                        if (M > 2) mm[g] = min(mm[g], (u32)u2[vv]);
+                                    }
+                                }
+#pragma unroll
+                                for (int g = 0; g < 4; ++g) {
+                                    const u32 bb = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
+                                    if (bb && res < 0) res = base - 32 * g - (__ffs(bb) - 1);
                                 }
                             }
-#pragma unroll
-                            for (int g = 0; g < 4; ++g) {
-                                const u32 bb = __ballot_sync(RIPS_FULL_MASK, mm[g] >= ks);
-                                if (bb && res < 0) res = base - 32 * g - (__ffs(bb) - 1);
-                            }
+                            if (lane == src) fv = res;
                         }
-                        if (lane == src) fv = res;
                     }
                 }
-                const bool found = fv >= 0;
-                const int vtop = (M > 2) ? vtop_slab : lv1;
-                const bool regular = found && fv > vtop;
+                finish(valid && !defer, keep, ci, key1, lv1, lx, fv);
                 const u32 kk = keep ? key1 - 1u : sentinel_key;
-                const u32 fvv = regular ? (u32)fv : (u32)n;
-                u64 prec = psentinel;
-                if (regular) {
-                    prec = SUM ? ci + ((u64)(u32)fv << p.tbits) + p.bt(fv, M + 1) : ci + sprec[fv];
-                    ++n_reg;
-                }
                 u64 rec = (u64)kk << lowbits;
                 if (keep) rec |= slab_low | (u64)((u32)lv1 * vmul + (u32)lx);
-                // ---- cofacet vertex below the top of s (whole rows of lanes: the columns holding the top vertices), or no
-                // cofacet of equal diameter: the facet test, the two small lists
-                if (__any_sync(RIPS_FULL_MASK, keep && !regular)) {
-                    bool is_irr = false, is_non = keep && !found;
-                    u64 irr_rec = 0;
-                    if (found && !regular) {
-                        int sv[M];
-                        sv[0] = lx;
-                        sv[1] = lv1;
-#pragma unroll
-                        for (int j = 2; j < M; ++j) sv[j] = v[j];
-                        int fseg = 0;
-#pragma unroll
-                        for (int j = 0; j < M; ++j) fseg += (sv[j] < fv) ? 1 : 0;
-                        if (s_is_youngest_facet<M, KT>(Kf, pitch, sv, key1, fv, fseg)) {
-                            irr_rec = (cofacet_index<M>(p.bt, sv, fv, fseg) << RIPS_PAIR_POS_BITS) | (u64)fseg;
-                            is_irr = true;
-                        } else
-                            is_non = true;
-                    }
-                    const u32 lt_mask = (1u << lane) - 1u;
-                    const u32 b_irr = __ballot_sync(RIPS_FULL_MASK, is_irr);
-                    if (b_irr) {
-                        u64 base = 0;
-                        if (lane == __ffs(b_irr) - 1)
-                            base = atomicAdd((unsigned long long*)(p.counters + S1C_IRREGULAR), (unsigned long long)__popc(b_irr));
-                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_irr) - 1) + __popc(b_irr & lt_mask);
-                        if (is_irr && base < p.irr_cap) p.irr_out[base] = irr_rec;
-                    }
-                    const u32 b_non = __ballot_sync(RIPS_FULL_MASK, is_non);
-                    if (b_non) {
-                        u64 base = 0;
-                        if (lane == __ffs(b_non) - 1)
-                            base = atomicAdd((unsigned long long*)(p.counters + S1C_NONAPP), (unsigned long long)__popc(b_non));
-                        base = __shfl_sync(RIPS_FULL_MASK, base, __ffs(b_non) - 1) + __popc(b_non & lt_mask);
-                        if (is_non && base < p.non_cap) p.non_out[base] = rec;
-                    }
-                }
                 // ---- stores and the fused histograms
                 if (valid) {
                     __stcs(p.cols_out + ci, rec);
-                    __stcs(p.pairs_out + ci, prec);
 #pragma unroll
                     for (int r = 0; r < S1_MAX_FUSED; ++r)
                         if (r < ncd) atomicAdd(&s_hist_cols[r][(kk >> (8 * r)) & 0xffu], 1u);
                 }
-#pragma unroll
-                for (int r = 0; r < S1_MAX_FUSED_P; ++r) {
-                    if (r < npd) { // few distinct digits in a warp: aggregate
-                        const u32 dg = valid ? ((fvv >> (8 * r)) & 0xffu) : 0xffffffffu;
-                        const u32 peers = __match_any_sync(RIPS_FULL_MASK, dg);
-                        if (valid && lane == __ffs(peers) - 1) atomicAdd(&s_hist_pairs[r][dg], (u32)__popc(peers));
-                    }
-                }
+                if (!SUM && qcnt >= 32) drain(32);
                 // ---- next pair, 32 positions further in the order e = C(v1, 2) + x
                 lx += 32;
                 xo += pitch32;
                 while (lx >= lv1) { lx -= lv1; xo -= r1o; ++lv1; r1o += pitch; }
             }
+            while (qcnt > 0) drain(qcnt < 32 ? qcnt : 32); // (the next slab has its own U2 row)
             idx += (u64)seg;
             rem -= seg;
             e0 += seg;
@@ -856,7 +927,7 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
     if (!p.compact && !p.count_only) {
         // slot mode: the leaner kernel, if its tables fit (C(., M+1) and one row of U2 per warp)
         const size_t u2rows = M > 2 ? (size_t)S1_WARPS * ((p.n + 7) & ~7) * sizeof(KT) : 0;
-        const size_t tables = (size_t)p.n * 8 + u2rows;
+        const size_t tables = (size_t)p.n * 8 + u2rows + 16 + (size_t)S1_WARPS * S1_QCAP * 16; // C(., M+1), U2 rows, the warps' queues (16-byte aligned)
 #ifdef RIPS_STRESS
         const size_t u2_limit = 8 * 1024; // beyond ~130 points the triangles and tetrahedra go to the general kernel (its slot mode with block maxima)
 #else
