@@ -936,7 +936,7 @@ cudaError_t launch_stage1_t(const Stage1Params& p, cudaStream_t st)
         if (p.Sf && u2rows <= u2_limit) return launch_persistent(enumerate_slot_kernel<M, KT, false, true>, p, u2rows, st);
         if (p.Sf && u2rows > u2_limit && u2_limit < 160 * 1024) return launch_persistent(enumerate_apparent_kernel<M, KT, false>, p, 0, st);
         if (kf_fits && kf_bytes + tables <= 190 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, true, false>, p, kf_bytes + tables, st);
-        if (tables <= 160 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, false>, p, tables, st);
+        if (tables <= 192 * 1024) return launch_persistent(enumerate_slot_kernel<M, KT, false, false>, p, tables, st); // (32 KB of it the queues: the same n as before them)
     }
     const int k_in = (!p.compact && !p.count_only && kf_fits) ? 1 : 0;
     const size_t smem = (k_in ? kf_bytes : 0) +
