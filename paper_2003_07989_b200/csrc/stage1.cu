@@ -499,8 +499,11 @@ __global__ void __launch_bounds__(S1_THREADS) enumerate_apparent_kernel(const St
 //     every cofacet test of the slab;
 //   * row offsets v1*pitch and x*pitch are carried along by lane_advance (additions only);
 //   * the cofacet scan tests the first four vertices n-1..n-4 of every lane at once, branch-free (the mean number of
-//     visits is about two: one lane-serial loop made the whole warp wait for its slowest lane), then four more for the
-//     warps that still have an open lane, then the warp-cooperative scan of the general kernel;
+//     visits is about two: one lane-serial loop made the whole warp wait for its slowest lane).  The lanes still open
+//     after that (one in ten) do not hold the step up: they put (cidx, key, v1, x) into a queue of their warp in shared
+//     memory, and the warp finishes 32 of them at a time (drain: twelve more vertices for every lane at once, the rest by
+//     the warp-cooperative scan, then the pair slot, the pair histogram and the small lists).  With block maxima (SUM:
+//     thousands of points, where the scans are the kernel) they are finished inside the step as in the general kernel;
 //   * digits of the fused histograms are taken from the 32-bit key / cofacet vertex, not from the 64-bit records;
 //   * C(v, M+1), the offset of a regular pair's row, comes from a copy of that binomial column in shared memory;
 //   * nothing is counted per warp step: the number of columns is total - over - cleared.
