@@ -172,6 +172,17 @@ def test_tiny_n(R, n):
     check_against_oracle(R, low + 1.0, n, 2, 0.5, f"n={n} below every distance")
 
 
+@pytest.mark.parametrize("n", [5, 8, 15, 16, 17, 20, 33, 47])
+def test_queue_of_open_scans_boundaries(R, n):
+    """The slot kernel's queue of open cofacet scans around its boundaries: fewer vertices than
+    a drained lane tests on its own (n < 16: no warp-cooperative scan at all), exactly as many, a few more (one partial
+    group of 32 behind them).  Random matrices: their scans are long, so most lanes are queued, the
+    queue fills and is drained in the middle of a slab, and many lanes are still open after the twelve vertices; the
+    matrix with heavy ties makes columns without any cofacet of equal diameter rare and irregular pairs common."""
+    check_against_oracle(R, inputs.random_matrix_lower(n, 400 + n), n, 3, inf, f"queue n={n} random matrix")
+    check_against_oracle(R, inputs.small_integer_lower(n, 500 + n, hi=3), n, 3, inf, f"queue n={n} ties")
+
+
 def test_threshold_sweep(R):
     w = inputs.config(1, 30)
     for q in (0.0, 0.1, 0.5, 0.9, 1.0):
